@@ -1,0 +1,419 @@
+"""Pins of the fp64 oracle against what the paper and the mathematics fix.
+
+None of these re-types the oracle's formula: each is a closed form with literal
+hand-computed numbers, a symmetry, a conservation law, an independent numerical
+integration, or a textbook special case.
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_binary, make_config
+
+P0 = dict(G=1.0, eps=0.0, gamma=0.0, beta=1.0, v_dead=0.0, tau_s=0.0, lens_mode=0)
+
+
+def _acc(x, m, *, v=None, star=None, R=(0.0, 0.0), **kw):
+    x = np.asarray(x, float)
+    v = np.zeros_like(x) if v is None else np.asarray(v, float)
+    star = np.zeros(len(x), np.int32) if star is None else star
+    return oracle.accel(x, v, np.asarray(m, float), star, R, dict(P0, **kw))
+
+
+# ---------------------------------------------------------------- P1: Eq. 4
+def test_p1_two_body_hand_sum():
+    # m1=1 at 0, m2=2 at x=3, eps=1: a1 = 2/(3+1)^2 = 0.125 toward +x,
+    # a2 = 1/16 = 0.0625 toward -x  (Eq. 4 divided by m_i)
+    a = _acc([[0, 0, 0], [3, 0, 0]], [1, 2], eps=1.0)
+    assert a[0] == pytest.approx([0.125, 0, 0], abs=1e-15)
+    assert a[1] == pytest.approx([-0.0625, 0, 0], abs=1e-15)
+
+
+def test_p1_collinear_unequal_masses_literal():
+    # x = 0,1,3  m = 1,2,4  G=2 eps=0.5 ; numbers worked by hand:
+    # a0 = 2*2/1.5^2 + 2*4/3.5^2 = 1.777777778 + 0.653061224 = 2.430839002
+    # a1 = -2*1/1.5^2 + 2*4/2.5^2 = -0.888888889 + 1.28 = 0.391111111
+    # a2 = -(2*1/3.5^2 + 2*2/2.5^2) = -(0.163265306 + 0.64) = -0.803265306
+    a = _acc([[0, 0, 0], [1, 0, 0], [3, 0, 0]], [1, 2, 4], G=2.0, eps=0.5)
+    assert a[:, 0] == pytest.approx([2.430839002, 0.391111111, -0.803265306], abs=2e-9)
+    assert np.abs(a[:, 1:]).max() == 0.0
+
+
+def test_p1_equilateral_and_tetrahedron_closed_forms():
+    L, eps, m, G = 2.0, 0.3, 0.7, 1.3
+    tri = np.array([[0, 0, 0], [L, 0, 0], [L / 2, L * math.sqrt(3) / 2, 0]])
+    a = _acc(tri, [m] * 3, G=G, eps=eps)
+    c = tri.mean(0)
+    mag = math.sqrt(3) * G * m / (L + eps) ** 2       # 2 cos30 = sqrt 3
+    for i in range(3):
+        u = (c - tri[i]) / np.linalg.norm(c - tri[i])
+        assert a[i] == pytest.approx(mag * u, abs=1e-14)
+    s = L / math.sqrt(8.0)                            # tetrahedron of edge L
+    tet = s * np.array([[1, 1, 1], [1, -1, -1], [-1, 1, -1], [-1, -1, 1]], float)
+    a = _acc(tet, [m] * 4, G=G, eps=eps)
+    mag = math.sqrt(6) * G * m / (L + eps) ** 2       # 3 * sqrt(2/3)
+    for i in range(4):
+        u = -tet[i] / np.linalg.norm(tet[i])
+        assert a[i] == pytest.approx(mag * u, abs=1e-14)
+
+
+def test_softening_is_r_plus_eps_squared_not_plummer():
+    # r=1, eps=0.5: (r+eps)^2 = 2.25 -> 0.4444...; Plummer (r^2+eps^2)^{3/2}*... would give 0.7155
+    a = _acc([[0, 0, 0], [0, 1, 0]], [1, 1], eps=0.5)
+    assert a[0, 1] == pytest.approx(1.0 / 2.25, abs=1e-15)
+
+
+def test_always_attractive_without_repulsion():
+    rng = np.random.default_rng(5)
+    x = rng.standard_normal((2, 3))
+    a = _acc(x, [1.0, 3.0], eps=0.01)
+    d = x[1] - x[0]
+    assert np.dot(a[0], d) > 0 and np.dot(a[1], -d) > 0
+
+
+# ------------------------------------------------- P2: displaced (lens) volume
+def test_p2_lens_volume_closed_form_limits():
+    R = 0.7
+    assert oracle.lens_volume(0.0, R) == pytest.approx(4.0 / 3.0 * math.pi * R ** 3, rel=1e-15)
+    assert abs(oracle.lens_volume(2 * R, R)) < 1e-15
+    h = 1e-6
+    slope = (oracle.lens_volume(2 * R, R) - oracle.lens_volume(2 * R - h, R)) / h
+    assert abs(slope) < 1e-5                                  # touches zero with zero slope
+    for r in (0.0, 0.35, 0.7, 1.05, 1.4):                    # factored form of the same cubic
+        fact = math.pi * (2 * R - r) ** 2 * (4 * R + r) / 12.0
+        assert oracle.lens_volume(r, R) == pytest.approx(fact, abs=1e-15)
+    # the literal printed r^2/12 form does NOT vanish at first contact (reading A1)
+    assert oracle.lens_volume(2.0, 1.0, 1) == pytest.approx(-math.pi / 3.0, rel=1e-12)
+
+
+def test_p2_lens_volume_is_sphere_sphere_overlap_monte_carlo():
+    # "proportional to the displaced volume": overlap of two radius-R balls
+    rng = np.random.default_rng(11)
+    R, n = 1.0, 2_000_000
+    g = rng.standard_normal((n, 3))
+    g /= np.linalg.norm(g, axis=1, keepdims=True)
+    p = g * np.cbrt(rng.random(n))[:, None] * R              # uniform in ball 1 at origin
+    for r in (0.4, 1.0, 1.6):
+        inside = np.linalg.norm(p - np.array([r, 0, 0]), axis=1) < R
+        vol = inside.mean() * 4.0 / 3.0 * math.pi * R ** 3
+        assert oracle.lens_volume(r, R) == pytest.approx(vol, rel=0, abs=6e-3)
+
+
+def test_rep_potential_is_integral_of_force():
+    R, g = 0.5, 7.0
+    assert abs(oracle.rep_potential(2 * R, R, g)) < 1e-15
+    for r in (0.1, 0.4, 0.8):
+        h = 1e-5
+        dU = (oracle.rep_potential(r + h, R, g) - oracle.rep_potential(r - h, R, g)) / (2 * h)
+        assert -dU == pytest.approx(g * oracle.lens_volume(r, R), rel=1e-8)
+
+
+# ------------------------------------------------------ P3 / A5: Eqs. 5 and 6
+def test_contact_hand_numbers_and_branch():
+    # G=0 isolates the repulsion. R=1, r=1: V = pi(4/3 - 1 + 1/12) = 5 pi/12 = 1.308996939
+    # gamma=3, m_i=2, m_j=5: converging a_i = 3*1.308996939/2 = 1.963495408 away from j,
+    # a_j = 3*1.308996939/5 = 0.785398163 away from i; diverging (beta=0.25) a quarter of that.
+    x = [[0, 0, 0], [1, 0, 0]]
+    kw = dict(G=0.0, gamma=3.0, beta=0.25, R=(1.0, 1.0))
+    a = _acc(x, [2, 5], v=[[0.1, 0, 0], [-0.1, 0, 0]], **kw)      # converging
+    assert a[:, 0] == pytest.approx([-1.963495408, 0.785398163], abs=1e-9)
+    a = _acc(x, [2, 5], v=[[-0.1, 0, 0], [0.1, 0, 0]], **kw)      # diverging
+    assert a[:, 0] == pytest.approx([-0.490873852, 0.196349541], abs=1e-9)
+    a = _acc(x, [2, 5], v=[[0, 1, 0], [0, 1, 0]], **kw)           # rdot == 0 -> gamma*beta (A5)
+    assert a[:, 0] == pytest.approx([-0.490873852, 0.196349541], abs=1e-9)
+    # dead band: rdot = -0.2 is converging only if v_dead < 0.2
+    v = [[0.1, 0, 0], [-0.1, 0, 0]]
+    assert _acc(x, [2, 5], v=v, v_dead=0.3, **kw)[0, 0] == pytest.approx(-0.490873852, abs=1e-9)
+    assert _acc(x, [2, 5], v=v, v_dead=0.1, **kw)[0, 0] == pytest.approx(-1.963495408, abs=1e-9)
+    # not in contact (r >= R_i + R_j): nothing
+    assert np.abs(_acc([[0, 0, 0], [2.0, 0, 0]], [2, 5], v=v, **kw)).max() == 0.0
+
+
+def test_cross_star_pair_uses_mean_radius():
+    # A2: R_i=0.6 (star 0), R_j=1.0 (star 1): contact iff r < 1.6, R_ij = 0.8
+    star = np.array([0, 1], np.int32)
+    kw = dict(G=0.0, gamma=1.0, beta=1.0, R=(0.6, 1.0), star=star)
+    assert np.abs(_acc([[0, 0, 0], [1.61, 0, 0]], [1, 1], **kw)).max() == 0.0
+    a = _acc([[0, 0, 0], [1.2, 0, 0]], [1, 1], **kw)
+    V = math.pi * (2 * 0.8 - 1.2) ** 2 * (4 * 0.8 + 1.2) / 12.0   # 0.184306...
+    assert a[0, 0] == pytest.approx(-V, rel=1e-12) and a[1, 0] == pytest.approx(V, rel=1e-12)
+
+
+def _head_on(beta, dt=2e-4, steps=6000):
+    R = 0.1
+    posm = np.array([[-0.15, 0, 0, 1.0], [0.15, 0, 0, 1.0]], np.float32)
+    vel = np.array([[0.5, 0, 0, 0], [-0.5, 0, 0, 0]], np.float32)
+    p = dict(P0, G=0.0, gamma=2.0e4, beta=beta, dt=dt, R_start=(R, R), R_end=(R, R), n_ramp=0)
+    s = oracle.Sim(posm, vel, np.zeros(2, np.int32), p)
+    s.step(steps)
+    return s
+
+
+def test_p3_restitution_elastic_iff_beta_one():
+    s = _head_on(1.0)
+    assert s.v[0, 0] == pytest.approx(-0.5, abs=2e-5) and s.v[1, 0] == pytest.approx(0.5, abs=2e-5)
+    s = _head_on(0.5)
+    e = abs(s.v[0, 0]) / 0.5                  # coefficient of restitution
+    # energy returned on the way out is beta times the energy stored on the way in
+    assert e == pytest.approx(math.sqrt(0.5), abs=2e-3)
+    assert s.x[0, 0] < -0.1 and s.x[1, 0] > 0.1   # they separated again
+
+
+# ----------------------------------------------- P4/P5/P6: invariants of a run
+@pytest.fixture(scope="module")
+def small_binary():
+    return make_binary(name="t", seed=7, n1=300, n2=212, shape="uniform", radius1=1.0,
+                       radius2=0.6, q=0.5, a=3.0, eps=0.01, dt=1e-3, nsteps=0,
+                       noise_frac=0.05, ramp_factor1=1.3, n_ramp=40)
+
+
+def test_p4_newtons_third_law(small_binary):
+    w = small_binary
+    m = w.posm[:, 3].astype(float)
+    a, kap, dl = oracle.accel(w.posm, w.vel, m, w.star, w.params["R_start"], w.params, want_diag=True)
+    net = np.linalg.norm((m[:, None] * a).sum(0))
+    assert net / (m * np.linalg.norm(a, axis=1)).sum() < 1e-13
+    assert (kap >= 1.0 - 1e-12).all()
+    # contacts do occur in this workload (otherwise the test above pins only gravity)
+    a0 = oracle.accel(w.posm, w.vel, m, w.star, w.params["R_start"], dict(w.params, gamma=0.0))
+    assert (np.linalg.norm(a - a0, axis=1) > 0).sum() > 50
+
+
+def test_p5_momentum_and_angular_momentum_conserved_with_contacts_and_ramp(small_binary):
+    w = small_binary
+    s = oracle.Sim(w.posm, w.vel, w.star, w.params)
+    e0 = s.energy()
+    s.step(80)                                 # crosses the end of the 40-step ramp
+    e1 = s.energy()
+    pscale = (s.m * np.linalg.norm(s.v, axis=1)).sum()
+    assert np.abs(e1["P"] - e0["P"]).max() / pscale < 1e-13
+    assert np.abs(e1["L"] - e0["L"]).max() / np.abs(e0["L"]).max() < 1e-13
+    assert s.n == 80
+    R = s.radii()
+    assert R[0] == pytest.approx(np.float32(w.params["R_end"][0]), rel=1e-7)
+
+
+def test_p6_energy_conserved_when_conservative_and_decreasing_when_inelastic(small_binary):
+    w = small_binary
+    base = dict(w.params, n_ramp=0, R_end=w.params["R_start"])
+
+    def drift(beta, dt, steps, gamma=None):
+        p = dict(base, beta=beta, dt=dt)
+        if gamma is not None:
+            p["gamma"] = gamma
+        s = oracle.Sim(w.posm, w.vel, w.star, p)
+        e0 = s.energy()["E"]
+        s.step(steps)
+        return (s.energy()["E"] - e0) / abs(e0)
+
+    d1 = drift(1.0, 1e-3, 40)
+    d2 = drift(1.0, 5e-4, 80)
+    assert abs(d1) < 1e-3                         # stiff contacts: (omega_c dt)^2 ~ 1e-2 of U_rep ripple
+    assert d1 / d2 == pytest.approx(4.0, rel=0.05)  # error ~ dt^2 over the same physical time
+    assert abs(drift(1.0, 1e-3, 40, gamma=0.0)) < 1e-6
+    assert drift(0.5, 1e-3, 40) < -10 * abs(d1)  # beta < 1 is an energy sink
+
+
+def test_force_is_minus_gradient_of_energy(small_binary):
+    # ties accel (Eqs. 4,5) to the potentials of orc_energy, whose gravity part is
+    # pinned by the two-body closed form below and repulsion part by A12's integral
+    w = small_binary
+    p = dict(w.params, beta=1.0, n_ramp=0, R_end=w.params["R_start"])
+    s = oracle.Sim(w.posm, w.vel, w.star, p)
+    a = s.accel()
+    U = lambda: s.energy()["Ug"] + s.energy()["Urep"]
+    h = 1e-6
+    for i, c in ((0, 0), (17, 1), (400, 2)):
+        x0 = s.x[i, c]
+        s.x[i, c] = x0 + h; up = U()
+        s.x[i, c] = x0 - h; um = U()
+        s.x[i, c] = x0
+        assert -(up - um) / (2 * h) / s.m[i] == pytest.approx(a[i, c], rel=2e-6, abs=1e-9)
+
+
+def test_two_body_potential_closed_form():
+    posm = np.array([[0, 0, 0, 2.0], [0, 4, 0, 3.0]], np.float32)
+    s = oracle.Sim(posm, np.zeros((2, 4), np.float32), np.zeros(2, np.int32),
+                   dict(P0, G=0.5, eps=1.0, dt=1.0, R_start=(0, 0), R_end=(0, 0), n_ramp=0))
+    assert s.energy()["Ug"] == pytest.approx(-0.5 * 2 * 3 / 5.0, rel=1e-15)   # -G m1 m2/(r+eps)
+
+
+# --------------------------------------- P7: circular two-body orbit, leapfrog
+def _two_body(a, eps, m1, m2, dt, steps):
+    M = m1 + m2
+    om = math.sqrt(M / (a * (a + eps) ** 2))      # G=1; softened circular frequency
+    posm = np.array([[-a * m2 / M, 0, 0, m1], [a * m1 / M, 0, 0, m2]])
+    vel = np.array([[0, -om * a * m2 / M, 0, 0], [0, om * a * m1 / M, 0, 0]])
+    s = oracle.Sim(posm, vel, np.zeros(2, np.int32),
+                   dict(P0, eps=eps, dt=dt, R_start=(0, 0), R_end=(0, 0), n_ramp=0))
+    s.x[:], s.v[:], s.m[:] = posm[:, :3], vel[:, :3], posm[:, 3]   # keep full double inputs
+    s.step(steps)
+    return s, posm, om
+
+
+@pytest.mark.parametrize("a,eps,M,T", [(3.0, 0.01, 1.5, 26.74616), (1.0, 0.1, 2.0, 4.887171),
+                                        (1.0, 0.0, 1.0, 2 * math.pi)])
+def test_p7_softened_circular_orbit_period_and_radius(a, eps, M, T):
+    assert 2 * math.pi * math.sqrt(a * (a + eps) ** 2 / M) == pytest.approx(T, rel=2e-7)
+    n = 10000
+    s, posm, om = _two_body(a, eps, M / 3, 2 * M / 3, T / n, n)
+    sep = np.linalg.norm(s.x[1] - s.x[0])
+    assert sep == pytest.approx(a, rel=1e-6)                       # radius constant
+    assert np.abs(s.x - posm[:, :3]).max() / a < 1e-4             # back at the start after T
+
+
+def test_leapfrog_is_second_order():
+    a, eps, M = 1.0, 0.1, 2.0
+    T = 2 * math.pi * math.sqrt(a * (a + eps) ** 2 / M)
+    errs = []
+    for n in (200, 400, 800):
+        s, posm, _ = _two_body(a, eps, 1.0, 1.0, T / n, n)
+        errs.append(np.abs(s.x - posm[:, :3]).max())
+    assert errs[0] / errs[1] == pytest.approx(4.0, rel=0.1)
+    assert errs[1] / errs[2] == pytest.approx(4.0, rel=0.1)
+
+
+# ------------------------------------------------- P8 / P9: Eq. 3 and L1
+EQ3_K06 = {0.3: 0.281031, 0.4: 0.303053, 0.5: 0.320788, 0.6: 0.335667, 0.8: 0.359772,
+           1.0: 0.378921, 2.5: 0.459873, 1 / 0.6: 0.423791, 1 / 0.3: 0.485382}
+EQ3_K069 = {0.3: 0.267237, 0.4: 0.287073, 1.0: 0.354265, 2.5: 0.424055}
+L1_DIST = {0.3: 0.620867, 0.4: 0.592948, 0.5: 0.570752, 0.6: 0.552343, 0.8: 0.522950, 1.0: 0.5}
+
+
+def test_p8_eq3_values():
+    for q, val in EQ3_K06.items():
+        assert oracle.roche_lobe_radius(q, 0.6) == pytest.approx(val, abs=1e-6)
+    for q, val in EQ3_K069.items():          # constant as printed
+        assert oracle.roche_lobe_radius(q, 0.69) == pytest.approx(val, abs=1e-6)
+    # hand evaluation at q=1: 0.49/(0.6 + ln 2) = 0.378921
+    assert oracle.roche_lobe_radius(1.0, 0.6) == pytest.approx(0.49 / (0.6 + math.log(2.0)), rel=1e-14)
+
+
+def _lobe_volume_radius(q_self_over_other: float) -> float:
+    """Volume-equivalent radius of the Roche lobe of the star whose mass is the
+    numerator, by direct numerical integration of the Roche potential (a=1,
+    G(M1+M2)=1): along each ray from the star, the lobe ends where the potential
+    first climbs back to its L1 value."""
+    qq = q_self_over_other
+    mu_s, mu_o = qq / (1 + qq), 1 / (1 + qq)       # this star at origin side
+    xs, xo = -mu_o, mu_s                           # barycentre at 0, separation 1
+    xl1 = xs + oracle.l1_distance(1.0 / qq)        # l1_distance(q) is measured from the primary of q=m2/m1
+
+    def phi(x, y, z):
+        r1 = np.sqrt((x - xs) ** 2 + y ** 2 + z ** 2)
+        r2 = np.sqrt((x - xo) ** 2 + y ** 2 + z ** 2)
+        return -mu_s / r1 - mu_o / r2 - 0.5 * (x ** 2 + y ** 2)
+
+    phi1 = phi(xl1, 0.0, 0.0)
+    nth, nph, nr = 96, 192, 1500
+    ct = (np.arange(nth) + 0.5) / nth * 2 - 1
+    ph = (np.arange(nph) + 0.5) / nph * 2 * math.pi
+    CT, PH = np.meshgrid(ct, ph, indexing="ij")
+    ST = np.sqrt(1 - CT ** 2)
+    ux, uy, uz = ST * np.cos(PH), ST * np.sin(PH), CT
+    rr = (np.arange(nr) + 0.5) / nr * (xl1 - xs) * 1.0001
+    inside = np.ones_like(ux, bool)
+    rmax = np.zeros_like(ux)
+    for r in rr:                                   # march outwards
+        inside &= phi(xs + r * ux, r * uy, r * uz) < phi1
+        rmax = np.where(inside, r, rmax)
+    vol = (rmax ** 3 / 3.0).mean() * 4 * math.pi
+    return (3 * vol / (4 * math.pi)) ** (1.0 / 3.0)
+
+
+@pytest.mark.parametrize("q", [0.4, 1.0, 2.5])
+def test_p8_eq3_against_integrated_lobe_volume(q):
+    rl = _lobe_volume_radius(q)
+    assert oracle.roche_lobe_radius(q, 0.6) == pytest.approx(rl, rel=0.01)          # standard constant
+    assert abs(oracle.roche_lobe_radius(q, 0.69) / rl - 1) > 0.04                    # printed 0.69 is off (A9)
+
+
+def test_p9_l1_location():
+    for q, d in L1_DIST.items():
+        assert oracle.l1_distance(q) == pytest.approx(d, abs=1e-6)
+    assert oracle.l1_distance(1.0) == pytest.approx(0.5, abs=1e-12)
+    # a massless element at L1 co-rotates: a + omega^2 x = 0 (omega^2 = G M / a^3, eps=gamma=0)
+    q, a = 0.4, 2.5
+    M1, M2 = 1.0, q
+    x1, x2 = -a * q / (1 + q), a / (1 + q)
+    xt = x1 + a * oracle.l1_distance(q)
+    acc = _acc([[x1, 0, 0], [x2, 0, 0], [xt, 0, 0]], [M1, M2, 1e-12])
+    om2 = (M1 + M2) / a ** 3
+    assert acc[2, 0] + om2 * xt == pytest.approx(0.0, abs=1e-9)
+
+
+def test_config3_ramp_factor_literal_matches_eq3():
+    from workloads.configs import CONFIG3_RAMP_FACTOR
+    q, a, R1 = 0.4, 2.5, 1.0
+    assert oracle.roche_lobe_radius(1 / q, 0.6) * a / R1 == pytest.approx(CONFIG3_RAMP_FACTOR, abs=1e-6)
+
+
+# ---------------------------------------------------------- P10: shell theorem
+def test_p10_shell_theorem_uniform_sphere():
+    w = make_binary(name="s", seed=3, n1=20000, n2=1, shape="uniform", radius1=1.0, radius2=0.1,
+                    q=1e-9, a=50.0, eps=1e-6, dt=1.0, nsteps=0, noise_frac=0.0, gamma=0.0)
+    x = w.posm[:-1, :3].astype(float)
+    c = x.mean(0)                       # centre of mass (equal masses): kills the dipole term
+    probes = np.array([[1.5, 0, 0], [0, -3.0, 0], [0, 0, 6.0]]) + c      # outside: GM/r^2
+    xx = np.concatenate([x, probes])
+    mm = np.concatenate([w.posm[:-1, 3].astype(float), np.full(len(probes), 1e-30)])
+    a = oracle.accel(xx, np.zeros_like(xx), mm, np.zeros(len(xx), np.int32), (0, 0),
+                     dict(P0, eps=1e-6))
+    for k, pr in enumerate(probes - c):
+        r = np.linalg.norm(pr)
+        assert a[len(x) + k] == pytest.approx(-pr / r ** 3, rel=0, abs=1e-2 / r ** 2)   # sampling quadrupole ~ N^-1/2 / r^4
+    # inside: the mean radial acceleration over a shell of elements is -G M r / R^3
+    d = x - c
+    r = np.linalg.norm(d, axis=1)
+    arad = (a[:len(x)] * d).sum(1) / r
+    for lo, hi in ((0.3, 0.4), (0.5, 0.6), (0.7, 0.8), (0.9, 1.0)):
+        sel = (r >= lo) & (r < hi)
+        assert sel.sum() > 500
+        assert arad[sel].mean() == pytest.approx(-r[sel].mean(), abs=0.02)
+
+
+# -------------------------------------------------------- expanding-star rule
+def test_radius_ramp_linear_in_step_count():
+    Rs, Re = (0.02, 0.03), (0.05, 0.03)
+    f32 = lambda v: float(np.float32(v))
+    assert oracle.radii(0, Rs, Re, 100)[0] == f32(0.02)
+    assert oracle.radii(50, Rs, Re, 100)[0] == f32(0.035)
+    assert oracle.radii(100, Rs, Re, 100)[0] == f32(0.05)
+    assert oracle.radii(1000, Rs, Re, 100)[0] == f32(0.05)       # stays at R_end
+    assert oracle.radii(7, Rs, Re, 100)[1] == f32(0.03)          # other star static
+    assert oracle.radii(7, Rs, Re, 0)[0] == f32(0.02)            # n_ramp=0: R = R_start
+    inc = np.diff([oracle.radii(n, Rs, Re, 100)[0] for n in range(101)])
+    assert np.allclose(inc, 0.0003, atol=1e-8)
+
+
+def test_kdk_uses_cached_acceleration_and_half_step_velocity():
+    # one step by hand for a two-body problem (A7): v_half = v0 + dt/2 a(x0); x1 = x0 + dt v_half;
+    # v1 = v_half + dt/2 a(x1)
+    posm = np.array([[0, 0, 0, 1.0], [2, 0, 0, 1.0]], np.float32)
+    vel = np.array([[0, 0.1, 0, 0], [0, -0.1, 0, 0]], np.float32)
+    p = dict(P0, eps=0.5, dt=0.25, R_start=(0, 0), R_end=(0, 0), n_ramp=0)
+    s = oracle.Sim(posm, vel, np.zeros(2, np.int32), p)
+    s.step(1)
+    a0 = 1 / 2.5 ** 2                                  # 0.16 toward each other
+    vhx = 0.125 * a0                                   # 0.02
+    x0 = 0.25 * vhx                                    # 0.005
+    assert s.x[0] == pytest.approx([x0, 0.025, 0], abs=1e-15)
+    d = np.array([2 - 2 * x0, -0.05, 0])
+    r = np.linalg.norm(d)
+    a1 = d / r / (r + 0.5) ** 2
+    assert s.v[0] == pytest.approx(np.array([vhx, 0.1, 0]) + 0.125 * a1, abs=1e-15)
+    # splitting a run into several calls changes nothing (cached acceleration)
+    s1 = oracle.Sim(posm, vel, np.zeros(2, np.int32), p); s1.step(6)
+    s2 = oracle.Sim(posm, vel, np.zeros(2, np.int32), p); s2.step(2); s2.step(4)
+    assert np.array_equal(s1.x, s2.x) and np.array_equal(s1.v, s2.v)
+
+
+def test_rows_subset_and_thread_count_independence():
+    w = make_config(1, scale=0.25)
+    m = w.posm[:, 3]
+    a = oracle.accel(w.posm, w.vel, m, w.star, w.params["R_start"], w.params)
+    rows = np.array([5, 0, 300, 511])
+    ar = oracle.accel(w.posm, w.vel, m, w.star, w.params["R_start"], w.params, rows=rows)
+    assert np.array_equal(a[rows], ar)
