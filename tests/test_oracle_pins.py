@@ -392,18 +392,18 @@ def test_kdk_uses_cached_acceleration_and_half_step_velocity():
     # one step by hand for a two-body problem (A7): v_half = v0 + dt/2 a(x0); x1 = x0 + dt v_half;
     # v1 = v_half + dt/2 a(x1)
     posm = np.array([[0, 0, 0, 1.0], [2, 0, 0, 1.0]], np.float32)
-    vel = np.array([[0, 0.1, 0, 0], [0, -0.1, 0, 0]], np.float32)
+    vel = np.array([[0, 0.125, 0, 0], [0, -0.125, 0, 0]], np.float32)   # exact in float32
     p = dict(P0, eps=0.5, dt=0.25, R_start=(0, 0), R_end=(0, 0), n_ramp=0)
     s = oracle.Sim(posm, vel, np.zeros(2, np.int32), p)
     s.step(1)
     a0 = 1 / 2.5 ** 2                                  # 0.16 toward each other
     vhx = 0.125 * a0                                   # 0.02
     x0 = 0.25 * vhx                                    # 0.005
-    assert s.x[0] == pytest.approx([x0, 0.025, 0], abs=1e-15)
-    d = np.array([2 - 2 * x0, -0.05, 0])
+    assert s.x[0] == pytest.approx([x0, 0.03125, 0], abs=1e-15)
+    d = np.array([2 - 2 * x0, -0.0625, 0])
     r = np.linalg.norm(d)
     a1 = d / r / (r + 0.5) ** 2
-    assert s.v[0] == pytest.approx(np.array([vhx, 0.1, 0]) + 0.125 * a1, abs=1e-15)
+    assert s.v[0] == pytest.approx(np.array([vhx, 0.125, 0]) + 0.125 * a1, abs=1e-15)
     # splitting a run into several calls changes nothing (cached acceleration)
     s1 = oracle.Sim(posm, vel, np.zeros(2, np.int32), p); s1.step(6)
     s2 = oracle.Sim(posm, vel, np.zeros(2, np.int32), p); s2.step(2); s2.step(4)
