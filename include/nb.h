@@ -1,0 +1,137 @@
+/*
+ * nb.h -- C ABI of the B200-native all-pairs binary-star element model.
+ *
+ * The hot path of arXiv 2303.12166 ("N-body simulation of binary star mass
+ * transfer using NVIDIA GPUs"): the O(N^2) pair-wise element-to-element
+ * acceleration (Eqs. 4-6; "the sum total of all the pair-wise
+ * element to element interactions") and the leapfrog step that
+ * consumes it, with the per-star expanding element radius
+ * (PAPER.md:60,89).  Every step of the path runs in hand-written sm_100a CUDA
+ * kernels (paper_2303_12166_b200/csrc); there is no CPU fallback.
+ *
+ * Conventions
+ *   - Every function returns NB_OK (0) or a negative nb_status; nothing aborts
+ *     or throws.  nb_strerror() gives the text; for NB_ECUDA, nb_last_cuda_error()
+ *     gives the cudaError_t.
+ *   - "dev" pointers are CUDA device pointers on the device that was current
+ *     at nb_create(); "host" pointers are ordinary host memory.
+ *   - The CALLER owns every device byte (state, output, workspace).  The
+ *     library owns only the host-side nb_ctx and never allocates device memory.
+ *     Borrowed pointers must stay valid until the next nb_set_state()/nb_destroy().
+ *   - All device work is enqueued on the borrowed stream given to nb_create().
+ *     Nothing synchronises except nb_set_state(), nb_energy() and
+ *     nb_download_state().  One ctx per host thread.
+ *   - Element layout: elements of star 0 first, then star 1.  posm[i] =
+ *     (x, y, z, m_i), vel[i] = (vx, vy, vz, unused); both float4, 16-byte aligned.
+ *
+ * Model (readings A1-A16 are listed in DESIGN.md):
+ *   d = x_j - x_i, r = |d|, R_ij = (R_star(i) + R_star(j))/2
+ *   a_i = sum_{j != i, r > 0} [ G m_j/(r+eps)^2 - (in contact: g*pi*V(r;R_ij)/m_i) ] d/r
+ *   in contact  <=> gamma > 0 and r < 2 R_ij
+ *   V(r;R) = 4/3 R^3 - R^2 r + r^3/12   (lens_mode 0: displaced volume, A1)
+ *          = 4/3 R^3 - R^2 r + r^2/12   (lens_mode 1: as printed)
+ *   g = gamma        if d.(v_j - v_i)/r < -v_dead   (converging, Eq. 5)
+ *     = gamma*beta   otherwise                      (diverging,  Eq. 6)
+ *   R_s(n) = R_start[s] + (R_end[s]-R_start[s]) * min(n, n_ramp)/n_ramp
+ *   step:  kick-drift-kick leapfrog, one force evaluation per step, a(x_{n+1})
+ *          evaluated with the half-step velocity (A7).
+ */
+#ifndef NB_H_
+#define NB_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nb_ctx nb_ctx;
+
+typedef enum {
+    NB_OK = 0,
+    NB_EINVAL = -1,   /* bad argument (null, n out of range, misaligned, bad parameter) */
+    NB_ESTATE = -2,   /* call order (no state set), or star[] not 0...0 1...1 */
+    NB_ECUDA = -3,    /* a CUDA call failed; see nb_last_cuda_error() */
+    NB_ENOMEM = -4,   /* workspace too small / host allocation failed */
+    NB_EARCH = -5     /* the current device is not sm_100 */
+} nb_status;
+
+typedef struct {
+    float G, eps, dt, q;        /* Eq. 4 G and eps; leapfrog step (89);
+                                   q = m2/m1 in (0,1] -- validated, metadata */
+    float gamma, beta;          /* Eqs. 5/6; gamma = 0 disables contact
+                                   terms; 0 < beta <= 1 */
+    float R_start[2], R_end[2]; /* element radius per star: expanding-star rule
+                                   (PAPER.md:89); equal => static */
+    int32_t n_ramp;             /* steps over which R goes start->end; 0 => R = R_start */
+    float v_dead;               /* converging iff rdot < -v_dead; 0 = literal rule (A5) */
+    int32_t lens_mode;          /* 0: r^3/12 displaced volume (A1); 1: r^2/12 as printed */
+} nb_params;
+
+/* Create a context for up to n_max elements.  `cuda_stream` is a cudaStream_t
+ * (NULL = the legacy default stream), borrowed.  Fails with NB_EARCH unless the
+ * current device has compute capability 10.x. */
+int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream);
+
+/* Bytes of device workspace nb_set_state() needs for a context of n_max elements
+ * (cached acceleration, split-j partial sums, device-side step/radius state,
+ * reduction scratch).  0 if n_max is out of range. */
+size_t nb_workspace_bytes(int64_t n_max);
+
+/* Bind the state.  posm, vel: dev float[n][4], 16-byte aligned, BORROWED and
+ * updated in place by nb_step().  star: dev int32[n], values 0...0 1...1 (checked
+ * on the device; read only during this call).  workspace: dev, 256-byte aligned,
+ * >= nb_workspace_bytes(n_max) bytes, BORROWED.  Resets the step count to 0 and
+ * drops the cached acceleration.  Synchronises the stream.  1 <= n <= n_max. */
+int nb_set_state(nb_ctx* ctx, int64_t n, float* posm, float* vel, const int32_t* star,
+                 void* workspace, size_t workspace_bytes);
+
+/* One evaluation of Eqs. 4-6 at the current (x, v, R(n)).  acc: dev float[n][4],
+ * caller-owned output, receives (ax, ay, az, 0).  Asynchronous on the stream. */
+int nb_compute_accel(nb_ctx* ctx, float* acc);
+
+/* nsteps leapfrog steps, asynchronous on the stream.  On
+ * completion of the stream work posm/vel hold (x_{n+nsteps}, v_{n+nsteps}),
+ * velocities synchronised with positions.  nsteps >= 0. */
+int nb_step(nb_ctx* ctx, int nsteps);
+
+/* Diagnostics at the current state, written to HOST out[12]:
+ * KE, U_grav, U_rep, E, Px, Py, Pz, Lx, Ly, Lz, |sum m_i a_i|, step count.
+ * U_grav = -sum_{i<j} G m_i m_j/(r+eps); U_rep per A12.  Synchronises the stream. */
+int nb_energy(nb_ctx* ctx, double* out);
+
+/* Current step count n and element radii R_s(n) (host outputs; either may be NULL).
+ * Synchronises the stream. */
+int nb_get_step(nb_ctx* ctx, int64_t* step, float* R);
+
+/* Host-buffer convenience for end-to-end use: copy host float[n][4] arrays into /
+ * out of the bound device buffers on the ctx stream.  Upload drops the cached
+ * acceleration and keeps the step count; download synchronises the stream.
+ * Pinned host memory makes the copies asynchronous.  Either pointer may be NULL. */
+int nb_upload_state(nb_ctx* ctx, const float* host_posm, const float* host_vel);
+int nb_download_state(nb_ctx* ctx, float* host_posm, float* host_vel);
+
+/* Launch configuration chosen for the bound state (for reports): i-elements per
+ * CTA, j-splits P, CTAs of the force kernel, CTAs of the update kernel. */
+int nb_get_launch_info(nb_ctx* ctx, int32_t* out4);
+
+/* Kernels launched by this ctx since nb_create() (for bench accounting). */
+int64_t nb_launch_count(nb_ctx* ctx);
+
+void nb_destroy(nb_ctx* ctx);
+const char* nb_strerror(int status);
+int nb_last_cuda_error(nb_ctx* ctx);
+
+/* Host-only scalars (no ctx).
+ * Eq. 3: Roche-lobe radius / separation of the star whose mass is
+ * the numerator of mass_ratio; k is the constant printed as 0.69 (standard 0.6, A9).
+ * nb_l1_distance: distance of L1 from the primary in units of the separation,
+ * q = m2/m1.  NaN on invalid arguments. */
+double nb_roche_lobe_radius(double mass_ratio, double k);
+double nb_l1_distance(double q);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NB_H_ */

@@ -1,0 +1,242 @@
+"""B200-native all-pairs binary-star element model (arXiv 2303.12166 hot path).
+
+Thin ctypes binding of the C ABI in include/nb.h: the functions below have the
+same names as the C entry points and only marshal arguments (torch tensors ->
+device pointers).  Every step of the path runs in the sm_100a CUDA kernels of
+csrc/; PyTorch is used for device memory and streams only.  There is no CPU
+fallback: if libnb.so is missing or no sm_100 device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Dict, Optional, Sequence
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libnb.so")
+
+NB_OK, NB_EINVAL, NB_ESTATE, NB_ECUDA, NB_ENOMEM, NB_EARCH = 0, -1, -2, -3, -4, -5
+
+EXPORTS = ("nb_create", "nb_workspace_bytes", "nb_set_state", "nb_compute_accel", "nb_step",
+           "nb_energy", "nb_get_step", "nb_upload_state", "nb_download_state",
+           "nb_get_launch_info", "nb_launch_count", "nb_destroy", "nb_strerror",
+           "nb_last_cuda_error", "nb_roche_lobe_radius", "nb_l1_distance")
+
+
+class nb_params(C.Structure):
+    """Mirror of `nb_params` in include/nb.h."""
+    _fields_ = [("G", C.c_float), ("eps", C.c_float), ("dt", C.c_float), ("q", C.c_float),
+                ("gamma", C.c_float), ("beta", C.c_float),
+                ("R_start", C.c_float * 2), ("R_end", C.c_float * 2),
+                ("n_ramp", C.c_int32), ("v_dead", C.c_float), ("lens_mode", C.c_int32)]
+
+
+class NbError(RuntimeError):
+    def __init__(self, status: int, where: str, cuda: int = 0):
+        self.status = status
+        msg = f"{where}: {nb_strerror(status)} (status {status})"
+        if status == NB_ECUDA:
+            msg += f", cudaError_t={cuda}"
+        super().__init__(msg)
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libnb.so (built by paper_2303_12166_b200.build); raises if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(
+                f"{LIB_PATH} is missing: build it with `python -m paper_2303_12166_b200.build` "
+                "(nvcc, sm_100a).  There is no CPU fallback.")
+        L = C.CDLL(LIB_PATH)
+        vp, i64, i32 = C.c_void_p, C.c_int64, C.c_int32
+        L.nb_create.restype = C.c_int
+        L.nb_create.argtypes = [C.POINTER(vp), i64, C.POINTER(nb_params), vp]
+        L.nb_workspace_bytes.restype = C.c_size_t
+        L.nb_workspace_bytes.argtypes = [i64]
+        L.nb_set_state.restype = C.c_int
+        L.nb_set_state.argtypes = [vp, i64, vp, vp, vp, vp, C.c_size_t]
+        L.nb_compute_accel.restype = C.c_int
+        L.nb_compute_accel.argtypes = [vp, vp]
+        L.nb_step.restype = C.c_int
+        L.nb_step.argtypes = [vp, C.c_int]
+        L.nb_energy.restype = C.c_int
+        L.nb_energy.argtypes = [vp, C.POINTER(C.c_double)]
+        L.nb_get_step.restype = C.c_int
+        L.nb_get_step.argtypes = [vp, C.POINTER(i64), C.POINTER(C.c_float)]
+        L.nb_upload_state.restype = C.c_int
+        L.nb_upload_state.argtypes = [vp, vp, vp]
+        L.nb_download_state.restype = C.c_int
+        L.nb_download_state.argtypes = [vp, vp, vp]
+        L.nb_get_launch_info.restype = C.c_int
+        L.nb_get_launch_info.argtypes = [vp, C.POINTER(i32)]
+        L.nb_launch_count.restype = i64
+        L.nb_launch_count.argtypes = [vp]
+        L.nb_destroy.restype = None
+        L.nb_destroy.argtypes = [vp]
+        L.nb_strerror.restype = C.c_char_p
+        L.nb_strerror.argtypes = [C.c_int]
+        L.nb_last_cuda_error.restype = C.c_int
+        L.nb_last_cuda_error.argtypes = [vp]
+        L.nb_roche_lobe_radius.restype = C.c_double
+        L.nb_roche_lobe_radius.argtypes = [C.c_double, C.c_double]
+        L.nb_l1_distance.restype = C.c_double
+        L.nb_l1_distance.argtypes = [C.c_double]
+        _lib = L
+    return _lib
+
+
+def _ptr(t) -> Optional[int]:
+    """Device/host address of a torch tensor, numpy array or raw int (None passes through)."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    return t.ctypes.data
+
+
+def make_params(p: Dict[str, object]) -> nb_params:
+    """nb_params from a dict with the keys of workloads.Workload.params."""
+    return nb_params(float(p["G"]), float(p["eps"]), float(p["dt"]), float(p["q"]),
+                     float(p.get("gamma", 0.0)), float(p.get("beta", 1.0)),
+                     (C.c_float * 2)(*[float(v) for v in p["R_start"]]),
+                     (C.c_float * 2)(*[float(v) for v in p["R_end"]]),
+                     int(p.get("n_ramp", 0)), float(p.get("v_dead", 0.0)), int(p.get("lens_mode", 0)))
+
+
+def _check(rc: int, where: str, ctx=None) -> None:
+    if rc != NB_OK:
+        raise NbError(rc, where, lib().nb_last_cuda_error(ctx) if ctx else 0)
+
+
+# ---- the C entry points, same names, argument marshalling only -------------------------------
+def nb_strerror(status: int) -> str:
+    return lib().nb_strerror(int(status)).decode()
+
+
+def nb_workspace_bytes(n_max: int) -> int:
+    return int(lib().nb_workspace_bytes(int(n_max)))
+
+
+def nb_create(n_max: int, params, cuda_stream: int = 0) -> int:
+    """Returns the ctx handle.  `cuda_stream`: raw cudaStream_t (torch stream .cuda_stream)."""
+    prm = params if isinstance(params, nb_params) else make_params(params)
+    ctx = C.c_void_p()
+    _check(lib().nb_create(C.byref(ctx), int(n_max), C.byref(prm), C.c_void_p(cuda_stream or None)),
+           "nb_create")
+    return ctx.value
+
+
+def nb_set_state(ctx: int, n: int, posm, vel, star, workspace, workspace_bytes: Optional[int] = None) -> None:
+    if workspace_bytes is None:
+        workspace_bytes = workspace.numel() * workspace.element_size()
+    _check(lib().nb_set_state(ctx, int(n), _ptr(posm), _ptr(vel), _ptr(star), _ptr(workspace),
+                              int(workspace_bytes)), "nb_set_state", ctx)
+
+
+def nb_compute_accel(ctx: int, acc) -> None:
+    _check(lib().nb_compute_accel(ctx, _ptr(acc)), "nb_compute_accel", ctx)
+
+
+def nb_step(ctx: int, nsteps: int) -> None:
+    _check(lib().nb_step(ctx, int(nsteps)), "nb_step", ctx)
+
+
+def nb_energy(ctx: int) -> Dict[str, object]:
+    out = (C.c_double * 12)()
+    _check(lib().nb_energy(ctx, out), "nb_energy", ctx)
+    v = list(out)
+    return dict(KE=v[0], Ug=v[1], Urep=v[2], E=v[3], P=v[4:7], L=v[7:10], Fnet=v[10], step=int(v[11]))
+
+
+def nb_get_step(ctx: int):
+    step = C.c_int64()
+    R = (C.c_float * 2)()
+    _check(lib().nb_get_step(ctx, C.byref(step), R), "nb_get_step", ctx)
+    return int(step.value), (float(R[0]), float(R[1]))
+
+
+def nb_upload_state(ctx: int, host_posm, host_vel) -> None:
+    _check(lib().nb_upload_state(ctx, _ptr(host_posm), _ptr(host_vel)), "nb_upload_state", ctx)
+
+
+def nb_download_state(ctx: int, host_posm, host_vel) -> None:
+    _check(lib().nb_download_state(ctx, _ptr(host_posm), _ptr(host_vel)), "nb_download_state", ctx)
+
+
+def nb_get_launch_info(ctx: int) -> Dict[str, int]:
+    out = (C.c_int32 * 4)()
+    _check(lib().nb_get_launch_info(ctx, out), "nb_get_launch_info", ctx)
+    return dict(i_per_cta=out[0], j_splits=out[1], force_ctas=out[2], update_ctas=out[3])
+
+
+def nb_launch_count(ctx: int) -> int:
+    return int(lib().nb_launch_count(ctx))
+
+
+def nb_destroy(ctx: int) -> None:
+    lib().nb_destroy(ctx)
+
+
+def nb_roche_lobe_radius(mass_ratio: float, k: float = 0.6) -> float:
+    return float(lib().nb_roche_lobe_radius(float(mass_ratio), float(k)))
+
+
+def nb_l1_distance(q: float) -> float:
+    return float(lib().nb_l1_distance(float(q)))
+
+
+class Simulation:
+    """Convenience owner of the device tensors one context borrows (torch allocates;
+    the kernels of libnb.so do all the work)."""
+
+    def __init__(self, posm, vel, star, params: Dict[str, object], device: str = "cuda:0",
+                 stream=None, n_max: Optional[int] = None):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2303_12166_b200 needs a CUDA (sm_100) device; there is no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.params = dict(params)
+        with torch.cuda.stream(self.stream):
+            self.posm = torch.as_tensor(posm, dtype=torch.float32).contiguous().to(self.device, copy=True)
+            self.vel = torch.as_tensor(vel, dtype=torch.float32).contiguous().to(self.device, copy=True)
+            self.star = torch.as_tensor(star, dtype=torch.int32).contiguous().to(self.device, copy=True)
+            self.n = int(self.posm.shape[0])
+            self.n_max = int(n_max or self.n)
+            self.workspace = torch.empty(nb_workspace_bytes(self.n_max), dtype=torch.uint8, device=self.device)
+            self.acc = torch.zeros((self.n, 4), dtype=torch.float32, device=self.device)
+        self.stream.synchronize()
+        self.ctx = nb_create(self.n_max, self.params, self.stream.cuda_stream)
+        nb_set_state(self.ctx, self.n, self.posm, self.vel, self.star, self.workspace)
+
+    def compute_accel(self):
+        nb_compute_accel(self.ctx, self.acc)
+        return self.acc
+
+    def step(self, nsteps: int = 1) -> None:
+        nb_step(self.ctx, nsteps)
+
+    def energy(self) -> Dict[str, object]:
+        return nb_energy(self.ctx)
+
+    def synchronize(self) -> None:
+        self.stream.synchronize()
+
+    def close(self) -> None:
+        if getattr(self, "ctx", None):
+            nb_destroy(self.ctx)
+            self.ctx = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,429 @@
+// nb_api.cu -- host side of the C ABI declared in include/nb.h.
+// Argument validation, launch configuration and kernel sequencing only; every
+// arithmetic step of the path runs in the kernels of nb_kernels.cuh.
+#include "nb.h"
+#include "nb_kernels.cuh"
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+using namespace nb;
+
+namespace {
+
+constexpr int64_t kMaxN = (int64_t)1 << 26;       // 67M elements: int indexing, n*TJ fits
+constexpr int kNumSMsFallback = 148;
+constexpr int kMomentBlocks = 296;
+constexpr size_t kAlign = 256;
+
+inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
+
+struct Plan {           // launch configuration of the force kernel for a given n
+    int I = 4;          // elements i per thread
+    int TJ = 256;       // j tile
+    int nib = 0;        // i blocks
+    int njt = 0;        // j tiles
+    int nsplit = 1;     // j splits P
+};
+
+// Upper bound on nsplit * n over all n <= n_max (partial-sum slab count).
+constexpr int64_t kTargetCtasPerSM = 48;
+
+Plan make_plan(int64_t n, int num_sms)
+{
+    Plan p;
+    if (n >= 16384)      { p.I = 4; p.TJ = 256; }
+    else                 { p.I = 2; p.TJ = 128; }
+    const int ib = kThreads * p.I;
+    p.nib = (int)((n + ib - 1) / ib);
+    p.njt = (int)((n + p.TJ - 1) / p.TJ);
+    // enough CTAs that the tail of the last wave is ~1/kTargetCtasPerSM of the run,
+    // but never less than 2 tiles per split
+    const int64_t target = (int64_t)num_sms * kTargetCtasPerSM;
+    int64_t P = (target + p.nib - 1) / p.nib;
+    const int64_t pmax = p.njt >= 2 ? p.njt / 2 : 1;
+    if (P > pmax) P = pmax;
+    if (P < 1) P = 1;
+    p.nsplit = (int)P;
+    return p;
+}
+
+int64_t partial_elems_bound(int64_t n_max)
+{
+    // nsplit <= target/nib + 1 with nib >= n/512  =>  nsplit*n <= 512*target + n, and
+    // nsplit <= njt/2 with TJ >= 128               =>  nsplit*n <= n^2/256 + n.
+    // Both grow with n, so the bound for n_max covers every n <= n_max.
+    const int64_t target = (int64_t)kNumSMsFallback * 2 * kTargetCtasPerSM;   // margin for > 148 SMs
+    const int64_t b1 = 512 * target + 2 * n_max;
+    const int64_t b2 = n_max * n_max / 256 + 2 * n_max;
+    return b1 < b2 ? b1 : b2;
+}
+
+struct Layout {
+    size_t off_dev, off_acc, off_part, off_red, total;
+};
+
+Layout make_layout(int64_t n_max)
+{
+    Layout L;
+    size_t o = 0;
+    L.off_dev = o;  o += align_up(sizeof(DevState));
+    L.off_acc = o;  o += align_up((size_t)n_max * sizeof(float4));
+    L.off_part = o; o += align_up((size_t)partial_elems_bound(n_max) * sizeof(float4));
+    const size_t pot_blocks = (size_t)((n_max + kThreads - 1) / kThreads);
+    const size_t red = (size_t)kMomentBlocks * kMomentCols * sizeof(double) + pot_blocks * 2 * sizeof(double);
+    L.off_red = o;  o += align_up(red);
+    L.total = o;
+    return L;
+}
+
+}  // namespace
+
+struct nb_ctx {
+    nb_params prm;
+    int64_t n_max = 0, n = 0;
+    int n1 = 0;
+    cudaStream_t stream = nullptr;
+    int num_sms = kNumSMsFallback;
+    float4* posm = nullptr;
+    float4* vel = nullptr;
+    char* ws = nullptr;
+    Layout lay{};
+    Plan plan{};
+    bool have_state = false, have_acc = false;
+    int last_cuda = 0;
+    int64_t launches = 0;
+
+    DevState* dev() const { return reinterpret_cast<DevState*>(ws + lay.off_dev); }
+    float4* acc() const { return reinterpret_cast<float4*>(ws + lay.off_acc); }
+    float4* part() const { return reinterpret_cast<float4*>(ws + lay.off_part); }
+    double* red() const { return reinterpret_cast<double*>(ws + lay.off_red); }
+};
+
+#define NB_CUDA(ctx, call)                                   \
+    do {                                                     \
+        cudaError_t e_ = (call);                             \
+        if (e_ != cudaSuccess) { (ctx)->last_cuda = (int)e_; return NB_ECUDA; } \
+    } while (0)
+
+namespace {
+
+bool params_ok(const nb_params* p)
+{
+    auto fin = [](float x) { return std::isfinite(x); };
+    if (!fin(p->G) || !fin(p->eps) || !fin(p->dt) || !fin(p->q) || !fin(p->gamma) || !fin(p->beta) ||
+        !fin(p->v_dead))
+        return false;
+    if (p->G < 0.f || p->eps < 0.f || p->dt < 0.f) return false;
+    if (!(p->q > 0.f && p->q <= 1.f)) return false;
+    if (p->gamma < 0.f) return false;
+    if (p->gamma > 0.f && !(p->beta > 0.f && p->beta <= 1.f)) return false;
+    if (p->v_dead < 0.f) return false;
+    if (p->n_ramp < 0) return false;
+    if (p->lens_mode != 0 && p->lens_mode != 1) return false;
+    for (int s = 0; s < 2; ++s)
+        if (!fin(p->R_start[s]) || !fin(p->R_end[s]) || p->R_start[s] < 0.f || p->R_end[s] < 0.f) return false;
+    return true;
+}
+
+template <int I, int TJ>
+int launch_force_t(nb_ctx* c, const ForceArgs& fa, int grid)
+{
+    if (c->prm.gamma > 0.f)
+        nb_force_kernel<I, TJ, true><<<grid, kThreads, 0, c->stream>>>(fa);
+    else
+        nb_force_kernel<I, TJ, false><<<grid, kThreads, 0, c->stream>>>(fa);
+    c->launches++;
+    NB_CUDA(c, cudaGetLastError());
+    return NB_OK;
+}
+
+// Row a2/a3: partial accelerations of all (i-block, j-split) pairs -> part[P][n]
+int launch_force(nb_ctx* c)
+{
+    ForceArgs fa;
+    fa.posm = c->posm; fa.vel = c->vel; fa.dev = c->dev(); fa.part = c->part();
+    fa.n = (int)c->n; fa.n1 = c->n1; fa.nib = c->plan.nib; fa.nsplit = c->plan.nsplit; fa.njt = c->plan.njt;
+    fa.G = c->prm.G; fa.eps = c->prm.eps;
+    fa.gamma = c->prm.gamma; fa.gamma_beta = c->prm.gamma * c->prm.beta;
+    fa.v_dead = c->prm.v_dead; fa.lens_mode = c->prm.lens_mode;
+    const int grid = c->plan.nib * c->plan.nsplit;
+    switch (c->plan.I) {
+        case 4: return launch_force_t<4, 256>(c, fa, grid);
+        default: return launch_force_t<2, 128>(c, fa, grid);
+    }
+}
+
+// Rows a4+a6+a5: reduce `nsrc` slabs of `src`, optionally store a, kick, drift, advance.
+int launch_update(nb_ctx* c, const float4* src, int nsrc, float4* acc_out, float kick_h, float drift_dt,
+                  int advance)
+{
+    UpdateArgs u;
+    u.src = src; u.acc_out = acc_out; u.posm = c->posm; u.vel = c->vel; u.dev = c->dev();
+    u.n = (int)c->n; u.nsrc = nsrc; u.kick_h = kick_h; u.drift_dt = drift_dt; u.advance = advance;
+    const int grid = (int)((c->n + 255) / 256);
+    nb_reduce_update_kernel<<<grid, 256, 0, c->stream>>>(u);
+    c->launches++;
+    NB_CUDA(c, cudaGetLastError());
+    return NB_OK;
+}
+
+int ensure_acc(nb_ctx* c)
+{
+    if (c->have_acc) return NB_OK;
+    int rc = launch_force(c);
+    if (rc) return rc;
+    rc = launch_update(c, c->part(), c->plan.nsplit, c->acc(), 0.f, 0.f, 0);
+    if (rc) return rc;
+    c->have_acc = true;
+    return NB_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* nb_strerror(int status)
+{
+    switch (status) {
+        case NB_OK: return "ok";
+        case NB_EINVAL: return "invalid argument";
+        case NB_ESTATE: return "invalid state or call order (no state bound, or star[] is not 0...0 1...1)";
+        case NB_ECUDA: return "CUDA error (see nb_last_cuda_error)";
+        case NB_ENOMEM: return "workspace too small or host allocation failed";
+        case NB_EARCH: return "device is not sm_100 (B200)";
+        default: return "unknown status";
+    }
+}
+
+int nb_last_cuda_error(nb_ctx* ctx) { return ctx ? ctx->last_cuda : 0; }
+
+size_t nb_workspace_bytes(int64_t n_max)
+{
+    if (n_max < 1 || n_max > kMaxN) return 0;
+    return make_layout(n_max).total;
+}
+
+int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream)
+{
+    if (!out) return NB_EINVAL;
+    *out = nullptr;
+    if (!p || n_max < 1 || n_max > kMaxN || !params_ok(p)) return NB_EINVAL;
+    int dev = 0, major = 0, sms = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return NB_ECUDA;
+    if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return NB_ECUDA;
+    if (major != 10) return NB_EARCH;
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return NB_ECUDA;
+    nb_ctx* c = new (std::nothrow) nb_ctx();
+    if (!c) return NB_ENOMEM;
+    c->prm = *p;
+    c->n_max = n_max;
+    c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+    c->num_sms = sms > 0 ? sms : kNumSMsFallback;
+    c->lay = make_layout(n_max);
+    *out = c;
+    return NB_OK;
+}
+
+void nb_destroy(nb_ctx* ctx) { delete ctx; }
+
+int nb_set_state(nb_ctx* c, int64_t n, float* posm, float* vel, const int32_t* star, void* workspace,
+                 size_t workspace_bytes)
+{
+    if (!c || !posm || !vel || !star || !workspace) return NB_EINVAL;
+    if (n < 1 || n > c->n_max) return NB_EINVAL;
+    if (((uintptr_t)posm & 15) || ((uintptr_t)vel & 15) || ((uintptr_t)star & 3) ||
+        ((uintptr_t)workspace & (kAlign - 1)))
+        return NB_EINVAL;
+    if (workspace_bytes < c->lay.total) return NB_ENOMEM;
+    c->have_state = false;
+    c->have_acc = false;
+    c->ws = static_cast<char*>(workspace);
+
+    DevState h;
+    std::memset(&h, 0, sizeof(h));
+    for (int s = 0; s < 2; ++s) {
+        h.R_start[s] = (double)c->prm.R_start[s];
+        h.R_end[s] = (double)c->prm.R_end[s];
+        h.R[s] = c->prm.R_start[s];
+    }
+    h.n_ramp = c->prm.n_ramp;
+    NB_CUDA(c, cudaMemcpyAsync(c->dev(), &h, sizeof(h), cudaMemcpyHostToDevice, c->stream));
+    nb_validate_star_kernel<<<c->num_sms, 256, 0, c->stream>>>(star, (int)n, c->dev());
+    c->launches++;
+    NB_CUDA(c, cudaGetLastError());
+    NB_CUDA(c, cudaMemcpyAsync(&h, c->dev(), sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (h.bad) return NB_ESTATE;
+
+    c->n = n;
+    c->n1 = h.n1;
+    c->posm = reinterpret_cast<float4*>(posm);
+    c->vel = reinterpret_cast<float4*>(vel);
+    c->plan = make_plan(n, c->num_sms);
+    if ((int64_t)c->plan.nsplit * n > partial_elems_bound(c->n_max)) return NB_ENOMEM;
+    c->have_state = true;
+    return NB_OK;
+}
+
+int nb_compute_accel(nb_ctx* c, float* acc)
+{
+    if (!c || !acc || ((uintptr_t)acc & 15)) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    int rc = launch_force(c);
+    if (rc) return rc;
+    rc = launch_update(c, c->part(), c->plan.nsplit, reinterpret_cast<float4*>(acc), 0.f, 0.f, 0);
+    if (rc) return rc;
+    if (reinterpret_cast<float4*>(acc) != c->acc()) {
+        NB_CUDA(c, cudaMemcpyAsync(c->acc(), acc, (size_t)c->n * sizeof(float4), cudaMemcpyDeviceToDevice,
+                                   c->stream));
+    }
+    c->have_acc = true;
+    return NB_OK;
+}
+
+int nb_step(nb_ctx* c, int nsteps)
+{
+    if (!c || nsteps < 0) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    if (nsteps == 0) return NB_OK;
+    const float dt = c->prm.dt;
+    int rc = ensure_acc(c);                                    // a(x_n) with v_n (A7)
+    if (rc) return rc;
+    // v_{n+1/2} = v_n + dt/2 a_n ; x_{n+1} = x_n + dt v_{n+1/2} ; n += 1, R(n)
+    rc = launch_update(c, c->acc(), 1, nullptr, 0.5f * dt, dt, 1);
+    if (rc) return rc;
+    for (int s = 1; s <= nsteps; ++s) {
+        rc = launch_force(c);                                  // a(x_{n+s}) with v_{n+s-1/2}
+        if (rc) return rc;
+        if (s < nsteps)   // two half kicks merged: v += dt a ; x += dt v ; advance
+            rc = launch_update(c, c->part(), c->plan.nsplit, nullptr, dt, dt, 1);
+        else              // closing half kick; cache a(x_{n+nsteps})
+            rc = launch_update(c, c->part(), c->plan.nsplit, c->acc(), 0.5f * dt, 0.f, 0);
+        if (rc) return rc;
+    }
+    c->have_acc = true;
+    return NB_OK;
+}
+
+int nb_get_step(nb_ctx* c, int64_t* step, float* R)
+{
+    if (!c) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    DevState h;
+    NB_CUDA(c, cudaMemcpyAsync(&h, c->dev(), sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (step) *step = h.step;
+    if (R) { R[0] = h.R[0]; R[1] = h.R[1]; }
+    return NB_OK;
+}
+
+int nb_energy(nb_ctx* c, double* out)
+{
+    if (!c || !out) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    int rc = ensure_acc(c);
+    if (rc) return rc;
+    const int n = (int)c->n;
+    double* red_m = c->red();
+    double* red_p = red_m + (size_t)kMomentBlocks * kMomentCols;
+    const int pot_blocks = (n + kThreads - 1) / kThreads;
+    nb_moments_kernel<<<kMomentBlocks, 256, 0, c->stream>>>(c->posm, c->vel, c->acc(), n, red_m);
+    c->launches++;
+    NB_CUDA(c, cudaGetLastError());
+    PotArgs pa;
+    pa.posm = c->posm; pa.dev = c->dev(); pa.out = red_p; pa.n = n; pa.n1 = c->n1;
+    pa.G = c->prm.G; pa.eps = c->prm.eps; pa.gamma = c->prm.gamma;
+    nb_potential_kernel<<<pot_blocks, kThreads, 0, c->stream>>>(pa);
+    c->launches++;
+    NB_CUDA(c, cudaGetLastError());
+
+    const size_t nd = (size_t)kMomentBlocks * kMomentCols + (size_t)pot_blocks * 2;
+    double* h = new (std::nothrow) double[nd];
+    if (!h) return NB_ENOMEM;
+    DevState hs;
+    cudaError_t e = cudaMemcpyAsync(h, red_m, nd * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(&hs, c->dev(), sizeof(hs), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess) { delete[] h; c->last_cuda = (int)e; return NB_ECUDA; }
+    double m[kMomentCols] = {0};
+    for (int b = 0; b < kMomentBlocks; ++b)
+        for (int k = 0; k < kMomentCols; ++k) m[k] += h[(size_t)b * kMomentCols + k];
+    double ug2 = 0.0, ur2 = 0.0;
+    const double* hp = h + (size_t)kMomentBlocks * kMomentCols;
+    for (int b = 0; b < pot_blocks; ++b) { ug2 += hp[2 * b]; ur2 += hp[2 * b + 1]; }
+    delete[] h;
+    out[0] = m[0];
+    out[1] = -0.5 * ug2;
+    out[2] = 0.5 * ur2;
+    out[3] = out[0] + out[1] + out[2];
+    for (int k = 0; k < 6; ++k) out[4 + k] = m[1 + k];
+    out[10] = std::sqrt(m[7] * m[7] + m[8] * m[8] + m[9] * m[9]);
+    out[11] = (double)hs.step;
+    return NB_OK;
+}
+
+int nb_upload_state(nb_ctx* c, const float* host_posm, const float* host_vel)
+{
+    if (!c) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    const size_t bytes = (size_t)c->n * sizeof(float4);
+    if (host_posm) NB_CUDA(c, cudaMemcpyAsync(c->posm, host_posm, bytes, cudaMemcpyHostToDevice, c->stream));
+    if (host_vel) NB_CUDA(c, cudaMemcpyAsync(c->vel, host_vel, bytes, cudaMemcpyHostToDevice, c->stream));
+    c->have_acc = false;
+    return NB_OK;
+}
+
+int nb_download_state(nb_ctx* c, float* host_posm, float* host_vel)
+{
+    if (!c) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    const size_t bytes = (size_t)c->n * sizeof(float4);
+    if (host_posm) NB_CUDA(c, cudaMemcpyAsync(host_posm, c->posm, bytes, cudaMemcpyDeviceToHost, c->stream));
+    if (host_vel) NB_CUDA(c, cudaMemcpyAsync(host_vel, c->vel, bytes, cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    return NB_OK;
+}
+
+int nb_get_launch_info(nb_ctx* c, int32_t* out4)
+{
+    if (!c || !out4) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    out4[0] = kThreads * c->plan.I;
+    out4[1] = c->plan.nsplit;
+    out4[2] = c->plan.nib * c->plan.nsplit;
+    out4[3] = (int)((c->n + 255) / 256);
+    return NB_OK;
+}
+
+int64_t nb_launch_count(nb_ctx* c) { return c ? c->launches : 0; }
+
+double nb_roche_lobe_radius(double mass_ratio, double k)
+{
+    if (!(mass_ratio > 0.0) || !std::isfinite(mass_ratio) || !(k > 0.0)) return NAN;
+    const double c = std::cbrt(mass_ratio);
+    return 0.49 * c * c / (k * c * c + std::log1p(c));           // Eq. 3
+}
+
+double nb_l1_distance(double q)
+{
+    if (!(q > 0.0) || !(q <= 1.0)) return NAN;
+    // Newton iteration on the co-rotating force balance along the line of centres
+    // (separation 1, G(m1+m2) = 1): s = distance from the primary m1.
+    const double mu2 = q / (1.0 + q), mu1 = 1.0 - mu2;
+    double s = 1.0 - std::cbrt(mu2 / 3.0);                        // Hill-radius start
+    for (int it = 0; it < 100; ++it) {
+        const double t = 1.0 - s;
+        const double f = -mu1 / (s * s) + mu2 / (t * t) + (s - mu2);
+        const double df = 2.0 * mu1 / (s * s * s) + 2.0 * mu2 / (t * t * t) + 1.0;
+        const double sn = s - f / df;
+        if (!(sn > 0.0 && sn < 1.0)) { s = 0.5 * (s + (sn <= 0.0 ? 0.0 : 1.0)); continue; }
+        if (std::fabs(sn - s) < 1e-15) { s = sn; break; }
+        s = sn;
+    }
+    return s;
+}
+
+}  // extern "C"

@@ -149,3 +149,18 @@ def make_config(idx: int, scale: Optional[float] = None) -> Workload:
         kw["n2"] = max(1, int(round(kw["n2"] * scale)))
         kw["name"] = f"{kw['name']}_x{scale:g}"
     return make_binary(**kw)
+
+
+def params_f32(params: Dict[str, object]) -> Dict[str, object]:
+    """The model parameters as the library holds them: every real rounded once to
+    float32 (returned as Python floats).  Feed THIS dict to both sides so that
+    a comparison never sees parameter rounding."""
+    f = lambda v: float(np.float32(v))
+    out = dict(params)
+    for k in ("G", "eps", "dt", "q", "gamma", "beta", "v_dead"):
+        if k in out:
+            out[k] = f(out[k])
+    for k in ("R_start", "R_end"):
+        if k in out:
+            out[k] = tuple(f(v) for v in out[k])
+    return out
