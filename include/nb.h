@@ -119,6 +119,12 @@ int nb_get_launch_info(nb_ctx* ctx, int32_t* out4);
 /* Kernels launched by this ctx since nb_create() (for bench accounting). */
 int64_t nb_launch_count(nb_ctx* ctx);
 
+/* Measurement aid: launch the all-pairs force kernel (row a2/a3 only; its partial
+ * sums land in the workspace and touch no state) `reps` times on the ctx stream
+ * after one warm-up launch, bracketed by CUDA events on that stream; HOST *ms_avg
+ * receives the average duration of one launch.  Synchronises the stream. */
+int nb_time_force_kernel(nb_ctx* ctx, int reps, float* ms_avg);
+
 void nb_destroy(nb_ctx* ctx);
 const char* nb_strerror(int status);
 int nb_last_cuda_error(nb_ctx* ctx);

@@ -36,6 +36,9 @@ Plan make_plan(int64_t n, int num_sms)
     Plan p;
     if (n >= 16384)      { p.I = 4; p.TJ = 256; }
     else                 { p.I = 2; p.TJ = 128; }
+#ifdef NB_FORCE_I2
+    p.I = 2; p.TJ = 128;
+#endif
     const int ib = kThreads * p.I;
     p.nib = (int)((n + ib - 1) / ib);
     p.njt = (int)((n + p.TJ - 1) / p.TJ);
@@ -399,6 +402,30 @@ int nb_get_launch_info(nb_ctx* c, int32_t* out4)
 }
 
 int64_t nb_launch_count(nb_ctx* c) { return c ? c->launches : 0; }
+
+int nb_time_force_kernel(nb_ctx* c, int reps, float* ms_avg)
+{
+    if (!c || !ms_avg || reps < 1) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    cudaEvent_t e0, e1;
+    NB_CUDA(c, cudaEventCreate(&e0));
+    NB_CUDA(c, cudaEventCreate(&e1));
+    int rc = launch_force(c);                                  // warm-up, untimed
+    if (rc == NB_OK) {
+        cudaEventRecord(e0, c->stream);
+        for (int r = 0; r < reps && rc == NB_OK; ++r) rc = launch_force(c);
+        cudaEventRecord(e1, c->stream);
+    }
+    cudaError_t e = cudaEventSynchronize(e1);
+    float ms = 0.f;
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    if (rc) return rc;
+    if (e != cudaSuccess) { c->last_cuda = (int)e; return NB_ECUDA; }
+    *ms_avg = ms / (float)reps;
+    return NB_OK;
+}
 
 double nb_roche_lobe_radius(double mass_ratio, double k)
 {

@@ -123,16 +123,25 @@ __device__ __forceinline__ void contact_term(const ForceArgs& a, int i, int j, f
 // with t = (r+eps)^2 >= eps^2 so the product cannot underflow.  That moves the
 // bound from the XU pipe (16 lanes/clk/SM) to the FMA pipe.
 // Per-tile fp32 partial sums are flushed into fp64 accumulators (short chains).
-// Contacts (CONTACT): candidates (min r^2 of the thread's pairs below the tile's
-// (R_i+R_j)^2 bound) are pushed, branch-free, to a small per-thread queue in
-// shared memory and resolved after the tile's loop by contact_term().
+// Contacts (CONTACT): the minimum r^2 over a group of kGroupJ elements j (FMNMX3 on
+// the ALU pipe) is tested once per group against the tile's (R_i+R_j)^2 bound;
+// candidate groups go to a small per-thread queue in shared memory and are
+// resolved after the tile's loop by contact_term().
 constexpr int kQueueDepth = 16;
+#ifndef NB_MINB4
+#define NB_MINB4 4      // resident CTAs/SM the I=4 kernel is compiled for (register cap 65536/(128*NB_MINB4))
+#endif
+#ifndef NB_UNROLL
+#define NB_UNROLL 4
+#endif
+constexpr int kGroupJ = NB_UNROLL;    // elements j per unrolled group = granularity of the contact test
 
 template <int I, int TJ, bool CONTACT>
-__global__ void __launch_bounds__(kThreads, (I >= 4 ? 4 : 6))
+__global__ void __launch_bounds__(kThreads, (I >= 4 ? NB_MINB4 : 6))
 nb_force_kernel(const __grid_constant__ ForceArgs a)
 {
-    static_assert(I % 2 == 0 && TJ % kThreads == 0 && TJ <= 256, "packed pairs; jj fits a byte");
+    static_assert(I % 2 == 0 && TJ % kThreads == 0 && TJ % kGroupJ == 0 && TJ / kGroupJ <= 256,
+                  "packed pairs; whole groups; group index fits a byte");
     constexpr int H = I / 2;                        // packed pairs per thread
     constexpr int LPT = TJ / kThreads;              // tile loads per thread
     __shared__ float4 sj[2][TJ];
@@ -216,41 +225,43 @@ nb_force_kernel(const __grid_constant__ ForceArgs a)
             const float D = Ri_max + Rj_max;
             rc2 = D * D;
         }
-        int qn = 0;                                  // candidates pushed in this tile
+        int qn = 0;                                  // candidate groups pushed in this tile
 
         const float4* __restrict__ s = sj[buf];
-#pragma unroll 4
-        for (int jj = 0; jj < TJ; ++jj) {
-            const float4 pj = s[jj];                 // LDS.128 broadcast
-            const f32x2 xj = pk2(pj.x, pj.x), yj = pk2(pj.y, pj.y), zj = pk2(pj.z, pj.z);
-            const f32x2 mj = pk2(pj.w, pj.w);
+#pragma unroll 1
+        for (int jg = 0; jg < TJ; jg += kGroupJ) {
             float rmin = 3.0e38f;
 #pragma unroll
-            for (int h = 0; h < H; ++h) {
-                const f32x2 dx = add2(xj, nxi[h]);
-                const f32x2 dy = add2(yj, nyi[h]);
-                const f32x2 dz = add2(zj, nzi[h]);
-                f32x2 r2 = fma2(dx, dx, tiny2);
-                r2 = fma2(dy, dy, r2);
-                r2 = fma2(dz, dz, r2);
-                float r2l, r2h;
-                unpk2(r2, r2l, r2h);
-                const f32x2 y = pk2(rsqrt_approx(r2l), rsqrt_approx(r2h));   // 1/r
-                const f32x2 sft = fma2(r2, y, eps2);                           // r + eps
-                const f32x2 tt = mul2(sft, sft);                               // (r+eps)^2
-                float tl, th;
-                unpk2(tt, tl, th);
-                const float ip = rcp_approx(tl * th);                          // one RCP for both lanes
-                const f32x2 u = pk2(ip * th, ip * tl);                         // 1/(r+eps)^2
-                const f32x2 c = mul2(mul2(mj, y), u);                          // G m_j/(r (r+eps)^2)  Eq. 4
-                ax[h] = fma2(c, dx, ax[h]);
-                ay[h] = fma2(c, dy, ay[h]);
-                az[h] = fma2(c, dz, az[h]);
-                if (CONTACT) rmin = fminf(rmin, fminf(r2l, r2h));
+            for (int u_ = 0; u_ < kGroupJ; ++u_) {
+                const float4 pj = s[jg + u_];            // LDS.128 broadcast
+                const f32x2 xj = pk2(pj.x, pj.x), yj = pk2(pj.y, pj.y), zj = pk2(pj.z, pj.z);
+#pragma unroll
+                for (int h = 0; h < H; ++h) {
+                    const f32x2 dx = add2(xj, nxi[h]);
+                    const f32x2 dy = add2(yj, nyi[h]);
+                    const f32x2 dz = add2(zj, nzi[h]);
+                    f32x2 r2 = fma2(dx, dx, tiny2);
+                    r2 = fma2(dy, dy, r2);
+                    r2 = fma2(dz, dz, r2);
+                    float r2l, r2h;
+                    unpk2(r2, r2l, r2h);
+                    const f32x2 y = pk2(rsqrt_approx(r2l), rsqrt_approx(r2h));   // 1/r
+                    const f32x2 sft = fma2(r2, y, eps2);                           // r + eps
+                    const f32x2 tt = mul2(sft, sft);                               // (r+eps)^2
+                    float tl, th;
+                    unpk2(tt, tl, th);
+                    const float ipm = rcp_approx(tl * th) * pj.w;                  // one RCP for both lanes
+                    const f32x2 um = pk2(ipm * th, ipm * tl);                      // G m_j/(r+eps)^2
+                    const f32x2 c = mul2(um, y);                                   // G m_j/(r (r+eps)^2)  Eq. 4
+                    ax[h] = fma2(c, dx, ax[h]);
+                    ay[h] = fma2(c, dy, ay[h]);
+                    az[h] = fma2(c, dz, az[h]);
+                    if (CONTACT) rmin = fminf(rmin, fminf(r2l, r2h));              // FMNMX3
+                }
             }
             if (CONTACT) {
-                if (rmin < rc2) {                    // rare (~5 I / N per j); compiles to predicated STS + IADD
-                    queue[(qn & (kQueueDepth - 1)) * kThreads + tid] = (unsigned char)jj;
+                if (rmin < rc2) {                    // rare: one branch per kGroupJ elements j
+                    queue[(qn & (kQueueDepth - 1)) * kThreads + tid] = (unsigned char)(jg / kGroupJ);
                     ++qn;
                 }
             }
@@ -265,26 +276,29 @@ nb_force_kernel(const __grid_constant__ ForceArgs a)
         }
 
         if (CONTACT && qn > 0) {
-            // Resolve this thread's candidates (all TJ elements if the queue overflowed).
+            // Resolve this thread's candidate groups (the whole tile if the queue overflowed).
             const bool all = qn > kQueueDepth;
-            const int cnt = all ? TJ : qn;
+            const int cnt = all ? TJ / kGroupJ : qn;
 #pragma unroll 1
             for (int q = 0; q < cnt; ++q) {
-                const int jj = all ? q : (int)queue[q * kThreads + tid];
-                const float4 pj = s[jj];
-                const int j = t * TJ + jj;
+                const int jg = kGroupJ * (all ? q : (int)queue[q * kThreads + tid]);
+#pragma unroll 1
+                for (int jj = jg; jj < jg + kGroupJ; ++jj) {
+                    const float4 pj = s[jj];
+                    const int j = t * TJ + jj;
 #pragma unroll
-                for (int h = 0; h < H; ++h) {
-                    float xl, xh, yl, yh, zl, zh;
-                    unpk2(nxi[h], xl, xh); unpk2(nyi[h], yl, yh); unpk2(nzi[h], zl, zh);
-                    const float dxl = pj.x + xl, dyl = pj.y + yl, dzl = pj.z + zl;
-                    const float dxh = pj.x + xh, dyh = pj.y + yh, dzh = pj.z + zh;
-                    if (fmaf(dzl, dzl, fmaf(dyl, dyl, dxl * dxl)) < rc2)
-                        contact_term(a, ibase + (2 * h) * kThreads, j, dxl, dyl, dzl, R0, R1,
-                                     accx[2 * h], accy[2 * h], accz[2 * h]);
-                    if (fmaf(dzh, dzh, fmaf(dyh, dyh, dxh * dxh)) < rc2)
-                        contact_term(a, ibase + (2 * h + 1) * kThreads, j, dxh, dyh, dzh, R0, R1,
-                                     accx[2 * h + 1], accy[2 * h + 1], accz[2 * h + 1]);
+                    for (int h = 0; h < H; ++h) {
+                        float xl, xh, yl, yh, zl, zh;
+                        unpk2(nxi[h], xl, xh); unpk2(nyi[h], yl, yh); unpk2(nzi[h], zl, zh);
+                        const float dxl = pj.x + xl, dyl = pj.y + yl, dzl = pj.z + zl;
+                        const float dxh = pj.x + xh, dyh = pj.y + yh, dzh = pj.z + zh;
+                        if (fmaf(dzl, dzl, fmaf(dyl, dyl, dxl * dxl)) < rc2)
+                            contact_term(a, ibase + (2 * h) * kThreads, j, dxl, dyl, dzl, R0, R1,
+                                         accx[2 * h], accy[2 * h], accz[2 * h]);
+                        if (fmaf(dzh, dzh, fmaf(dyh, dyh, dxh * dxh)) < rc2)
+                            contact_term(a, ibase + (2 * h + 1) * kThreads, j, dxh, dyh, dzh, R0, R1,
+                                         accx[2 * h + 1], accy[2 * h + 1], accz[2 * h + 1]);
+                    }
                 }
             }
         }

@@ -1,0 +1,379 @@
+"""Parity of the CUDA path (through the C ABI) with the fp64 oracle, element by
+element on the same seeded float32 inputs.  Tolerances (BASELINE.json north_star):
+accelerations max |a_gpu - a_oracle| / |a_oracle| <= 2e-5 (plus the A6 allowance
+Delta_i for pairs sitting on the converging/diverging switch); positions after
+10 steps max |dx_i| / a <= 1e-4 (A15).
+"""
+import hashlib
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_binary, make_config, params_f32
+
+pytestmark = pytest.mark.gpu
+
+ACC_TOL = 2.0e-5
+POS_TOL = 1.0e-4
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+def _sim(nb, w, p=None, **kw):
+    return nb.Simulation(w.posm, w.vel, w.star, p or params_f32(w.params), **kw)
+
+
+def _gpu_accel(nb, w, p):
+    s = _sim(nb, w, p)
+    a = s.compute_accel()
+    s.synchronize()
+    out = a.cpu().numpy().astype(np.float64)
+    info = nb.nb_get_launch_info(s.ctx)
+    s.close()
+    assert (out[:, 3] == 0).all()
+    return out[:, :3], info
+
+
+def _check_accel(nb, w, p=None, rows=None, tol=ACC_TOL):
+    p = p or params_f32(w.params)
+    a_gpu, info = _gpu_accel(nb, w, p)
+    assert np.isfinite(a_gpu).all()
+    a_or, kap, dl = oracle.accel(w.posm, w.vel, w.posm[:, 3], w.star, p["R_start"], p, rows=rows, want_diag=True)
+    sel = np.arange(w.n) if rows is None else rows
+    err = np.linalg.norm(a_gpu[sel] - a_or, axis=1)
+    an = np.linalg.norm(a_or, axis=1)
+    ok = an > 0
+    rel = np.maximum(err[ok] - dl[ok], 0.0) / an[ok]
+    assert rel.max() <= tol, f"max rel err {rel.max():.3e} (kappa {kap[ok][np.argmax(rel)]:.1f}) launch {info}"
+    assert (err[~ok] <= 1e-12).all()
+    # A6: only a sliver of the ~5 contact pairs per element sits within tau_s of the switch
+    # (tau_s / sigma_rdot ~ 1e-4 of them); anything more means the dead band is not doing its job
+    assert (dl > 0).sum() <= 3 + 1e-3 * 5 * len(sel)
+    return a_gpu, rel.max()
+
+
+def _sample(n, k, seed):
+    return np.sort(np.random.default_rng(seed).choice(n, min(k, n), replace=False))
+
+
+# ------------------------------------------------------------ accelerations
+@pytest.mark.parametrize("idx", [1, 2])
+def test_accel_full_parity_small_configs(nb, idx):
+    _check_accel(nb, make_config(idx))
+
+
+@pytest.mark.parametrize("idx,nrows", [(3, 4096), (4, 2048), (5, 1024)])
+def test_accel_sampled_parity_full_size_configs(nb, idx, nrows):
+    """BASELINE full sizes in the launch configuration bench.py times; the oracle
+    computes a seeded sample of rows one by one against all N elements."""
+    w = make_config(idx)
+    a_gpu, _ = _check_accel(nb, w, rows=_sample(w.n, nrows, 77 + idx))
+    # property that holds at any size: Newton's third law (P4), fp32 level
+    m = w.posm[:, 3].astype(np.float64)
+    net = np.linalg.norm((m[:, None] * a_gpu).sum(0))
+    assert net / (m * np.linalg.norm(a_gpu, axis=1)).sum() < 1e-5
+
+
+@pytest.mark.parametrize("n1,n2", [(1000, 777), (1, 1), (3, 0), (0, 5), (129, 1), (255, 257), (5000, 4321),
+                                    (16384, 1), (17000, 3001)])
+def test_accel_ragged_and_degenerate_sizes(nb, n1, n2):
+    """Sizes that are not multiples of the 128/256/512 tiles, a single star, one element."""
+    kw = dict(name="r", seed=5, n1=max(n1, 1), n2=max(n2, 1), shape="uniform", radius1=1.0, radius2=0.6,
+              q=0.5, a=3.0, eps=0.01, dt=1e-3, nsteps=0)
+    w = make_binary(**kw)
+    if n1 == 0:                                  # only star 1
+        keep = slice(1, None)
+    elif n2 == 0:                                # only star 0
+        keep = slice(0, n1)
+    else:
+        keep = slice(None)
+    w.posm, w.vel, w.star = w.posm[keep].copy(), w.vel[keep].copy(), w.star[keep].copy()
+    assert w.n == n1 + n2
+    _check_accel(nb, w)
+
+
+def test_single_element_has_zero_acceleration(nb):
+    w = make_binary(name="one", seed=1, n1=1, n2=1, shape="uniform", radius1=1.0, radius2=1.0, q=1.0, a=2.0,
+                    eps=0.1, dt=1e-3, nsteps=0)
+    w.posm, w.vel, w.star = w.posm[:1].copy(), w.vel[:1].copy(), w.star[:1].copy()
+    a, _ = _gpu_accel(nb, w, params_f32(w.params))
+    assert (a == 0).all()
+
+
+@pytest.mark.parametrize("override", [dict(gamma=0.0), dict(lens_mode=1), dict(beta=1.0), dict(v_dead=0.0),
+                                       dict(eps=0.0), dict(G=0.0), dict(G=2.5, eps=0.05)])
+def test_accel_parameter_variants(nb, override):
+    w = make_config(1)
+    w.vel[:, :3] += np.random.default_rng(3).standard_normal((w.n, 3)).astype(np.float32) * 0.03
+    p = params_f32(dict(w.params, **override))
+    _check_accel(nb, w, p)
+
+
+def test_contact_branches_both_occur_and_match(nb):
+    """Eq. 5 and Eq. 6 pairs both present (velocity noise); compare the contact part alone."""
+    w = make_config(2, scale=0.25)
+    p = params_f32(w.params)
+    a1, _ = _gpu_accel(nb, w, p)
+    a0, _ = _gpu_accel(nb, w, dict(p, gamma=0.0))
+    o1 = oracle.accel(w.posm, w.vel, w.posm[:, 3], w.star, p["R_start"], p)
+    o0 = oracle.accel(w.posm, w.vel, w.posm[:, 3], w.star, p["R_start"], dict(p, gamma=0.0))
+    touched = np.linalg.norm(o1 - o0, axis=1) > 0
+    assert touched.sum() > 100
+    assert ((np.linalg.norm(a1 - a0, axis=1) > 0) == touched).mean() > 0.999
+    d_gpu, d_or = (a1 - a0)[touched], (o1 - o0)[touched]
+    assert np.linalg.norm(d_gpu - d_or, axis=1).max() <= 2e-5 * np.linalg.norm(o1[touched], axis=1).max()
+
+
+def test_cross_star_contact_radius(nb):
+    """A2: two elements of different stars touch iff r < R_0 + R_1."""
+    posm = np.array([[0, 0, 0, 1.0], [1.2, 0, 0, 1.0]], np.float32)
+    vel = np.zeros((2, 4), np.float32)
+    star = np.array([0, 1], np.int32)
+    p = params_f32(dict(G=0.0, eps=0.0, dt=1e-3, q=1.0, gamma=1.0, beta=1.0, R_start=(0.6, 1.0), R_end=(0.6, 1.0),
+                        n_ramp=0, v_dead=0.0, lens_mode=0))
+    s = nb.Simulation(posm, vel, star, p)
+    a = s.compute_accel().cpu().numpy().astype(np.float64)
+    o = oracle.accel(posm, vel, posm[:, 3], star, p["R_start"], p)
+    assert a[0, 0] < 0 and np.allclose(a[:, :3], o, rtol=2e-6, atol=0)
+    posm[1, 0] = 1.61
+    s2 = nb.Simulation(posm, vel, star, p)
+    assert (s2.compute_accel().cpu().numpy() == 0).all()
+
+
+# ------------------------------------------------------------- trajectories
+def _check_traj(nb, w, nsteps=10, chunks=None):
+    p = params_f32(w.params)
+    o = oracle.Sim(w.posm, w.vel, w.star, p)
+    o.step(nsteps)
+    s = _sim(nb, w, p)
+    for c in (chunks or [nsteps]):
+        s.step(c)
+    s.synchronize()
+    x = s.posm.cpu().numpy().astype(np.float64)
+    v = s.vel.cpu().numpy().astype(np.float64)
+    step, R = nb.nb_get_step(s.ctx)
+    s.close()
+    assert step == nsteps
+    assert np.allclose(R, o.radii(), rtol=0, atol=0), (R, o.radii())
+    assert np.array_equal(x[:, 3], w.posm[:, 3].astype(np.float64))           # masses untouched
+    perr = np.linalg.norm(x[:, :3] - o.x, axis=1).max() / w.meta["a"]
+    vscale = w.meta["omega"] * w.meta["a"]
+    verr = np.linalg.norm(v[:, :3] - o.v, axis=1).max() / vscale
+    assert perr <= POS_TOL, perr
+    assert verr <= 1e-2, verr        # velocities carry dt * (contact-switch) differences; positions are the bar
+    return perr, verr
+
+
+def test_ten_step_trajectory_config1(nb):
+    perr, _ = _check_traj(nb, make_config(1))
+    assert perr < 1e-5
+
+
+def test_ten_step_trajectory_config2_with_noise(nb):
+    _check_traj(nb, make_config(2))
+
+
+def test_ten_step_trajectory_with_radius_ramp(nb):
+    """Config 3's recipe at 1/8 size with the ramp compressed into 8 steps, so the 10
+    steps cross the end of the ramp; radii are compared bit for bit."""
+    w = make_config(3, scale=0.125)
+    w.params["n_ramp"] = 8
+    _check_traj(nb, w)
+
+
+def test_step_calls_can_be_split(nb):
+    """nb_step(10) vs nb_step(3)+nb_step(7): same steps; only the merged dt-kick vs two
+    dt/2 kicks differ, by fp32 rounding."""
+    w = make_config(1)
+    p = params_f32(w.params)
+    a, b = _sim(nb, w, p), _sim(nb, w, p)
+    a.step(10)
+    b.step(3); b.step(7)
+    a.synchronize(); b.synchronize()
+    xa, xb = a.posm.cpu().numpy(), b.posm.cpu().numpy()
+    assert np.abs(xa - xb).max() < 5e-6
+    _check_traj(nb, w, chunks=[1] * 10)
+
+
+def _golden(idx):
+    path = os.path.join(GOLDEN, f"config{idx}_step10_sample.txt")
+    if not os.path.exists(path):
+        pytest.skip(f"{path} not generated")
+    head = open(path).read(600)
+    sha = head.split("sha256=")[1].split()[0]
+    return np.loadtxt(path), sha
+
+
+@pytest.mark.parametrize("idx", [3, 4])
+def test_ten_step_trajectory_full_size_against_stored_oracle(nb, idx):
+    """Configs 3 (N=65,536, with the ramp) and 4 (N=262,144, headline): positions after 10
+    steps against the oracle's, stored by tests/golden/make_golden.py for 1,024 elements."""
+    gold, sha = _golden(idx)
+    w = make_config(idx)
+    h = hashlib.sha256()
+    h.update(np.ascontiguousarray(w.posm).tobytes()); h.update(np.ascontiguousarray(w.vel).tobytes())
+    assert h.hexdigest() == sha, "workload differs from the one the stored values belong to"
+    s = _sim(nb, w)
+    s.step(10)
+    s.synchronize()
+    x = s.posm.cpu().numpy().astype(np.float64)
+    v = s.vel.cpu().numpy().astype(np.float64)
+    e = s.energy()
+    s.close()
+    rows = gold[:, 0].astype(np.int64)
+    perr = np.linalg.norm(x[rows, :3] - gold[:, 1:4], axis=1).max() / w.meta["a"]
+    verr = np.linalg.norm(v[rows, :3] - gold[:, 4:7], axis=1).max() / (w.meta["omega"] * w.meta["a"])
+    assert perr <= POS_TOL, perr
+    assert verr <= 1e-2, verr
+    assert np.isfinite(x).all() and np.isfinite(v).all() and e["step"] == 10
+
+
+def test_one_step_consistency_at_full_size_config5(nb):
+    """N = 1,048,576: the oracle checks one leapfrog step for a sample of elements, given the
+    GPU's own states before and after (x1 = x0 + dt (v0 + dt/2 a(x0)))."""
+    w = make_config(5)
+    p = params_f32(w.params)
+    rows = _sample(w.n, 512, 9)
+    s = _sim(nb, w, p)
+    s.step(1)
+    s.synchronize()
+    x1 = s.posm.cpu().numpy().astype(np.float64)[:, :3]
+    v1 = s.vel.cpu().numpy().astype(np.float64)[:, :3]
+    s.close()
+    dt = p["dt"]
+    a0 = oracle.accel(w.posm, w.vel, w.posm[:, 3], w.star, p["R_start"], p, rows=rows)
+    vh = w.vel[rows, :3].astype(np.float64) + 0.5 * dt * a0
+    xo = w.posm[rows, :3].astype(np.float64) + dt * vh
+    assert np.linalg.norm(x1[rows] - xo, axis=1).max() / w.meta["a"] < 1e-6
+    # a(x1) with the half-step velocities the GPU used (reconstructed to fp32 accuracy)
+    vhalf_all = (x1 - w.posm[:, :3].astype(np.float64)) / dt
+    a1 = oracle.accel(x1, vhalf_all, w.posm[:, 3], w.star, p["R_start"], p, rows=rows)
+    vo = vh + 0.5 * dt * a1
+    assert np.abs(v1[rows] - vo).max() / (w.meta["omega"] * w.meta["a"]) < 1e-3
+
+
+# ------------------------------------------------------ diagnostics, invariants
+def test_energy_and_momenta_match_oracle(nb):
+    w = make_config(1)
+    p = params_f32(w.params)
+    s = _sim(nb, w, p)
+    e = s.energy()
+    o = oracle.Sim(w.posm, w.vel, w.star, p).energy()
+    for k in ("KE", "Ug", "Urep", "E"):
+        assert e[k] == pytest.approx(o[k], rel=2e-6), k
+    assert np.allclose(e["P"], o["P"], atol=1e-7) and np.allclose(e["L"], o["L"], rtol=1e-6, atol=1e-7)
+    assert e["Fnet"] < 1e-5 * 30 and e["step"] == 0
+    s.step(5)
+    e5, _ = s.energy(), o
+    oo = oracle.Sim(w.posm, w.vel, w.star, p); oo.step(5)
+    assert e5["E"] == pytest.approx(oo.energy()["E"], rel=1e-5) and e5["step"] == 5
+    s.close()
+
+
+def test_long_run_invariants_config1(nb):
+    """P5/A16: leapfrog with pairwise central forces keeps P and L; E does not grow (beta < 1)."""
+    w = make_config(1)
+    s = _sim(nb, w)
+    e0 = s.energy()
+    s.step(300)
+    e1 = s.energy()
+    x = s.posm.cpu().numpy()
+    s.close()
+    assert np.isfinite(x).all()
+    pscale = float((w.posm[:, 3] * np.linalg.norm(w.vel[:, :3], axis=1)).sum())
+    assert np.abs(np.array(e1["P"]) - np.array(e0["P"])).max() / pscale < 1e-5
+    assert abs(e1["L"][2] - e0["L"][2]) / abs(e0["L"][2]) < 1e-5
+    assert e1["E"] < e0["E"] + 1e-4 * abs(e0["E"])
+    assert e1["step"] == 300
+
+
+def test_results_are_bitwise_reproducible(nb):
+    w = make_config(2, scale=0.5)
+    outs = []
+    for _ in range(2):
+        s = _sim(nb, w)
+        s.step(3)
+        a = s.compute_accel()
+        s.synchronize()
+        outs.append((s.posm.cpu().numpy().copy(), a.cpu().numpy().copy()))
+        s.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+
+
+# ------------------------------------------------------------------ boundary
+def test_upload_download_and_restart(nb):
+    import torch
+    w = make_config(1)
+    p = params_f32(w.params)
+    s = _sim(nb, w, p)
+    s.step(2)
+    hp = torch.empty((w.n, 4), dtype=torch.float32).pin_memory()
+    hv = torch.empty((w.n, 4), dtype=torch.float32).pin_memory()
+    nb.nb_download_state(s.ctx, hp, hv)
+    assert torch.equal(hp, s.posm.cpu()) and torch.equal(hv, s.vel.cpu())
+    # restart a second context from the downloaded state: same continuation
+    s2 = nb.Simulation(w.posm, w.vel, w.star, p)
+    nb.nb_upload_state(s2.ctx, hp, hv)
+    s.step(2); s2.step(2)
+    s.synchronize(); s2.synchronize()
+    # s continues with the cached a(x_2), which saw the half-step velocity (A7); s2 re-evaluates
+    # a(x_2) with the synchronised v_2, so a few contact pairs near the switch take the other branch
+    d = np.abs(s.posm.cpu().numpy() - s2.posm.cpu().numpy()).max(axis=1)
+    assert np.quantile(d, 0.9) < 1e-6 and d.max() < 1e-3
+    s.close(); s2.close()
+
+
+def test_error_codes(nb):
+    import torch
+    w = make_config(1, scale=0.125)
+    p = params_f32(w.params)
+    dev = torch.device("cuda:0")
+    posm = torch.tensor(w.posm, device=dev); vel = torch.tensor(w.vel, device=dev)
+    star = torch.tensor(w.star, device=dev)
+    ws = torch.empty(nb.nb_workspace_bytes(w.n), dtype=torch.uint8, device=dev)
+    acc = torch.empty((w.n, 4), dtype=torch.float32, device=dev)
+    L = nb.lib()
+    for bad in (dict(q=0.0), dict(q=1.5), dict(beta=0.0), dict(beta=1.5), dict(eps=-1.0), dict(gamma=-1.0),
+                dict(lens_mode=3), dict(n_ramp=-1), dict(dt=float("nan")), dict(R_start=(-0.1, 0.1))):
+        with pytest.raises(nb.NbError) as ei:
+            nb.nb_create(w.n, dict(p, **bad))
+        assert ei.value.status == nb.NB_EINVAL
+    with pytest.raises(nb.NbError):
+        nb.nb_create(0, p)
+    ctx = nb.nb_create(w.n, p, torch.cuda.current_stream().cuda_stream)
+    assert L.nb_compute_accel(ctx, acc.data_ptr()) == nb.NB_ESTATE          # no state yet
+    assert L.nb_step(ctx, 1) == nb.NB_ESTATE
+    args = (posm.data_ptr(), vel.data_ptr(), star.data_ptr(), ws.data_ptr(), ws.numel())
+    assert L.nb_set_state(ctx, w.n + 1, *args) == nb.NB_EINVAL               # n > n_max
+    assert L.nb_set_state(ctx, 0, *args) == nb.NB_EINVAL
+    assert L.nb_set_state(ctx, w.n, None, *args[1:]) == nb.NB_EINVAL          # null
+    assert L.nb_set_state(ctx, w.n, posm.data_ptr() + 4, *args[1:]) == nb.NB_EINVAL   # misaligned
+    assert L.nb_set_state(ctx, w.n, *args[:4], 1024) == nb.NB_ENOMEM          # workspace too small
+    bad_star = star.clone(); bad_star[0] = 1                                  # 1 0 0 ... : not star-0-first
+    assert L.nb_set_state(ctx, w.n, args[0], args[1], bad_star.data_ptr(), args[3], args[4]) == nb.NB_ESTATE
+    bad_star[0] = 7
+    assert L.nb_set_state(ctx, w.n, args[0], args[1], bad_star.data_ptr(), args[3], args[4]) == nb.NB_ESTATE
+    assert L.nb_compute_accel(ctx, acc.data_ptr()) == nb.NB_ESTATE            # failed bind leaves no state
+    assert L.nb_set_state(ctx, w.n, *args) == nb.NB_OK
+    assert L.nb_compute_accel(ctx, None) == nb.NB_EINVAL
+    assert L.nb_step(ctx, -1) == nb.NB_EINVAL
+    assert L.nb_step(ctx, 0) == nb.NB_OK
+    assert L.nb_compute_accel(ctx, acc.data_ptr()) == nb.NB_OK
+    torch.cuda.synchronize()
+    assert torch.isfinite(acc).all()
+    assert nb.nb_launch_count(ctx) >= 3
+    nb.nb_destroy(ctx)
+
+
+def test_runs_on_a_side_stream(nb):
+    import torch
+    w = make_config(1)
+    st = torch.cuda.Stream()
+    s = nb.Simulation(w.posm, w.vel, w.star, params_f32(w.params), stream=st)
+    s.step(2)
+    st.synchronize()
+    ref = _sim(nb, w); ref.step(2); ref.synchronize()
+    assert torch.equal(s.posm, ref.posm)
+    assert nb.nb_time_force_kernel(s.ctx, 2) > 0
+    s.close(); ref.close()
