@@ -105,12 +105,17 @@ int nb_energy(nb_ctx* ctx, double* out);
  * Synchronises the stream. */
 int nb_get_step(nb_ctx* ctx, int64_t* step, float* R);
 
-/* Host-buffer convenience for end-to-end use: copy host float[n][4] arrays into /
- * out of the bound device buffers on the ctx stream.  Upload drops the cached
- * acceleration and keeps the step count; download synchronises the stream.
- * Pinned host memory makes the copies asynchronous.  Either pointer may be NULL. */
-int nb_upload_state(nb_ctx* ctx, const float* host_posm, const float* host_vel);
-int nb_download_state(nb_ctx* ctx, float* host_posm, float* host_vel);
+/* Host-buffer entry points for end-to-end use and checkpoint/restart: copy HOST
+ * float[n][4] arrays into / out of the bound device buffers on the ctx stream.
+ * The full state of a run is (x, v, a(x_n), n): host_acc carries the cached
+ * acceleration (the one the next nb_step() starts from, which saw the half-step
+ * velocity, A7).  Upload with host_acc == NULL drops the cache, so the next step
+ * re-evaluates a(x_n) with the uploaded velocities; the step count is kept.
+ * Download with host_acc != NULL evaluates a(x_n) first if it is not cached.
+ * Download synchronises the stream.  Pinned host memory makes the copies
+ * asynchronous.  Any pointer may be NULL (skipped). */
+int nb_upload_state(nb_ctx* ctx, const float* host_posm, const float* host_vel, const float* host_acc);
+int nb_download_state(nb_ctx* ctx, float* host_posm, float* host_vel, float* host_acc);
 
 /* Launch configuration chosen for the bound state (for reports): i-elements per
  * CTA, j-splits P, CTAs of the force kernel, CTAs of the update kernel. */

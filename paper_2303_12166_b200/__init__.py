@@ -68,9 +68,9 @@ def lib() -> C.CDLL:
         L.nb_get_step.restype = C.c_int
         L.nb_get_step.argtypes = [vp, C.POINTER(i64), C.POINTER(C.c_float)]
         L.nb_upload_state.restype = C.c_int
-        L.nb_upload_state.argtypes = [vp, vp, vp]
+        L.nb_upload_state.argtypes = [vp, vp, vp, vp]
         L.nb_download_state.restype = C.c_int
-        L.nb_download_state.argtypes = [vp, vp, vp]
+        L.nb_download_state.argtypes = [vp, vp, vp, vp]
         L.nb_get_launch_info.restype = C.c_int
         L.nb_get_launch_info.argtypes = [vp, C.POINTER(i32)]
         L.nb_launch_count.restype = i64
@@ -163,12 +163,13 @@ def nb_get_step(ctx: int):
     return int(step.value), (float(R[0]), float(R[1]))
 
 
-def nb_upload_state(ctx: int, host_posm, host_vel) -> None:
-    _check(lib().nb_upload_state(ctx, _ptr(host_posm), _ptr(host_vel)), "nb_upload_state", ctx)
+def nb_upload_state(ctx: int, host_posm, host_vel, host_acc=None) -> None:
+    _check(lib().nb_upload_state(ctx, _ptr(host_posm), _ptr(host_vel), _ptr(host_acc)), "nb_upload_state", ctx)
 
 
-def nb_download_state(ctx: int, host_posm, host_vel) -> None:
-    _check(lib().nb_download_state(ctx, _ptr(host_posm), _ptr(host_vel)), "nb_download_state", ctx)
+def nb_download_state(ctx: int, host_posm, host_vel, host_acc=None) -> None:
+    _check(lib().nb_download_state(ctx, _ptr(host_posm), _ptr(host_vel), _ptr(host_acc)),
+           "nb_download_state", ctx)
 
 
 def nb_get_launch_info(ctx: int) -> Dict[str, int]:

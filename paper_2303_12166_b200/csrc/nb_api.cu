@@ -368,22 +368,28 @@ int nb_energy(nb_ctx* c, double* out)
     return NB_OK;
 }
 
-int nb_upload_state(nb_ctx* c, const float* host_posm, const float* host_vel)
+int nb_upload_state(nb_ctx* c, const float* host_posm, const float* host_vel, const float* host_acc)
 {
     if (!c) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
     const size_t bytes = (size_t)c->n * sizeof(float4);
     if (host_posm) NB_CUDA(c, cudaMemcpyAsync(c->posm, host_posm, bytes, cudaMemcpyHostToDevice, c->stream));
     if (host_vel) NB_CUDA(c, cudaMemcpyAsync(c->vel, host_vel, bytes, cudaMemcpyHostToDevice, c->stream));
-    c->have_acc = false;
+    if (host_acc) NB_CUDA(c, cudaMemcpyAsync(c->acc(), host_acc, bytes, cudaMemcpyHostToDevice, c->stream));
+    c->have_acc = host_acc != nullptr;
     return NB_OK;
 }
 
-int nb_download_state(nb_ctx* c, float* host_posm, float* host_vel)
+int nb_download_state(nb_ctx* c, float* host_posm, float* host_vel, float* host_acc)
 {
     if (!c) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
     const size_t bytes = (size_t)c->n * sizeof(float4);
+    if (host_acc) {
+        const int rc = ensure_acc(c);
+        if (rc) return rc;
+        NB_CUDA(c, cudaMemcpyAsync(host_acc, c->acc(), bytes, cudaMemcpyDeviceToHost, c->stream));
+    }
     if (host_posm) NB_CUDA(c, cudaMemcpyAsync(host_posm, c->posm, bytes, cudaMemcpyDeviceToHost, c->stream));
     if (host_vel) NB_CUDA(c, cudaMemcpyAsync(host_vel, c->vel, bytes, cudaMemcpyDeviceToHost, c->stream));
     NB_CUDA(c, cudaStreamSynchronize(c->stream));

@@ -1,0 +1,68 @@
+"""Host logic of bench.py without a GPU: the reference arm prints a contract-shaped
+JSON line, and the max/sum-over-ranks timing reduction works across 2 ranks (gloo)."""
+import json
+import os
+import subprocess
+import sys
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_reference_arm_prints_contract_line():
+    env = dict(os.environ, PYTHONPATH=ROOT)
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
+                          "--warmup", "1"], capture_output=True, text=True, env=env, cwd=ROOT, timeout=600)
+    assert out.returncode == 0, out.stderr
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["unit"] == "interactions/s" and line["value"] > 1e6
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] >= 1
+    assert line["e2e"] == {"value": line["value"], "unit": line["unit"], "h2d_bytes_per_step": 0,
+                           "d2h_bytes_per_step": 0}
+    assert line["config"]["workload"].startswith("config4") and line["higher_is_better"] is True
+
+
+def test_own_arm_refuses_to_run_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1", "--warmup", "0"],
+                         capture_output=True, text=True, cwd=ROOT, timeout=600)
+    assert out.returncode != 0 and "no CPU fallback" in (out.stderr + out.stdout)
+
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, {root!r})
+import bench
+rank, world = bench.dist_init("gloo")
+bench.barrier()
+mx = bench.reduce_over_ranks(10.0 + 5.0 * rank, "max")
+sm = bench.reduce_over_ranks(1.0 + rank, "sum")
+print(f"RESULT {{rank}} {{world}} {{mx}} {{sm}}", flush=True)
+# rank-0-only reference arm: other ranks exit 0 without work
+if rank != 0:
+    class A: gpus=2; steps=1; warmup=1
+    assert bench.run_reference(A) == 0
+import torch.distributed as dist
+dist.destroy_process_group()
+"""
+
+
+def test_two_rank_gloo_timing_reduction(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER.format(root=ROOT))
+    procs = []
+    for r in range(2):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE="2", MASTER_ADDR="127.0.0.1",
+                   MASTER_PORT="29617")
+        procs.append(subprocess.Popen([sys.executable, str(script)], stdout=subprocess.PIPE,
+                                      stderr=subprocess.PIPE, text=True, env=env))
+    outs = [p.communicate(timeout=300) for p in procs]
+    for p, (so, se) in zip(procs, outs):
+        assert p.returncode == 0, se
+    for r, (so, _) in enumerate(outs):
+        res = [l for l in so.splitlines() if l.startswith("RESULT")][0].split()
+        assert int(res[1]) == r and int(res[2]) == 2
+        assert float(res[3]) == 15.0 and float(res[4]) == 3.0        # max over ranks, sum over ranks

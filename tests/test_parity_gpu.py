@@ -321,7 +321,15 @@ def test_upload_download_and_restart(nb):
     # a(x_2) with the synchronised v_2, so a few contact pairs near the switch take the other branch
     d = np.abs(s.posm.cpu().numpy() - s2.posm.cpu().numpy()).max(axis=1)
     assert np.quantile(d, 0.9) < 1e-6 and d.max() < 1e-3
-    s.close(); s2.close()
+    # with the cached acceleration carried along, (x, v, a, n) is the full state: bitwise continuation
+    ha = torch.empty((w.n, 4), dtype=torch.float32).pin_memory()
+    nb.nb_download_state(s.ctx, hp, hv, ha)
+    s3 = nb.Simulation(w.posm, w.vel, w.star, p)
+    nb.nb_upload_state(s3.ctx, hp, hv, ha)
+    s.step(3); s3.step(3)
+    s.synchronize(); s3.synchronize()
+    assert torch.equal(s.posm, s3.posm) and torch.equal(s.vel, s3.vel)
+    s.close(); s2.close(); s3.close()
 
 
 def test_error_codes(nb):
