@@ -44,7 +44,7 @@ FLOP_PER_INTERACTION = 21          # 19 FMA-pipe flop + rsqrt + 
 FP32_LANES_PER_SM = 128
 BENCH_CONFIG = 4                   # BASELINE.json configs[3]: the headline throughput config
 L2_FLUSH_BYTES = 256 << 20         # > 126 MB L2
-CPU_SAMPLE_ROWS = 8192             # cpu_baseline: rows x N fp64 pair evaluations
+CPU_SAMPLE_ROWS = 32768            # cpu_baseline: rows x N fp64 pair evaluations (~10-60 core-seconds)
 REF_ROWS_PER_STEP = 2048           # --impl reference: rows x N per "step"
 
 
