@@ -13,7 +13,7 @@ DESIGN.md).  interactions = N^2 ordered pairs per step.
              nb_step(1); L2 flushed between steps; max over ranks.
   e2e        the same step through the C ABI with HOST (pinned) buffers: H2D of
              (x, v, a) + nb_step(1) + D2H of (x, v, a) inside the timed region.
-  roofline   the force kernel alone (nb_time_force_kernel: events on its stream)
+  roofline   the all-pairs gravity kernel alone (nb_time_force_kernel: events on its stream)
              against the FP32 CUDA-core peak  SMs x 128 lanes x 2 flop x max clock,
              with the stated 21 flop / interaction convention ("alu" bound).
   cpu_baseline  the fp64 oracle (oracle/, as it stands) on the box's host cores, on a
@@ -239,8 +239,9 @@ def run_own(args):
     ms_total = reduce_over_ranks(ms_local, "max", dev)
     value = float(n) * n * args.steps * world / (ms_total * 1e-3)
 
-    # ---- roofline of the dominant kernel (force), timed alone on its stream
+    # ---- roofline of the dominant kernel (all-pairs gravity), timed alone on its stream
     k_ms = nb.nb_time_force_kernel(sim.ctx, max(3, min(args.steps, 10)))
+    c_ms = nb.nb_time_contact_pass(sim.ctx, max(3, min(args.steps, 10)))
     props = torch.cuda.get_device_properties(dev)
     sm_max_mhz = clocks.get("sm_max_mhz") or 1965.0
     peak_tflops = props.multi_processor_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
@@ -248,8 +249,9 @@ def run_own(args):
     step_ms = ms_total / args.steps
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved / peak_tflops, "traffic": ncu_traffic_bytes(),
-                "kernel": "nb_force_kernel<4,256,true>", "kernel_ms": k_ms,
+                "kernel": "nb_gravity_kernel<2,256>", "kernel_ms": k_ms,
                 "kernel_share_of_step": k_ms / step_ms,
+                "contact_pass_ms": c_ms, "contact_pass_share_of_step": c_ms / step_ms,
                 "interactions_per_s": float(n) * n / (k_ms * 1e-3),
                 "flop_per_interaction": FLOP_PER_INTERACTION,
                 "peak_source": f"derived: {props.multi_processor_count} SMs x 128 FP32 lanes x 2 flop x "
@@ -299,7 +301,7 @@ def run_own(args):
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
             "config": {"workload": w.name, "n": n, "n1": w.meta["n1"], "n2": w.meta["n2"], "q": p["q"],
                        "eps": p["eps"], "dt": p["dt"], "gamma": p["gamma"], "beta": p["beta"],
-                       "step": "KDK leapfrog: kick/drift + all-pairs force + split-j reduce/kick",
+                       "step": "KDK leapfrog: kick/drift + contact pass (Eqs. 5/6) + all-pairs gravity (Eq. 4) + reduce/kick",
                        "l2": "flushed between timed steps (256 MiB fill)", "parallelism": "replicas only",
                        "launch": info},
             "steps_per_s": 1e3 / step_ms,

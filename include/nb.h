@@ -76,7 +76,8 @@ int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream
 
 /* Bytes of device workspace nb_set_state() needs for a context of n_max elements
  * (cached acceleration, split-j partial sums, device-side step/radius state,
- * reduction scratch).  0 if n_max is out of range. */
+ * reduction scratch, and the contact pass's Hilbert keys, sort scratch, ordered copy and
+ * group boxes).  0 if n_max is out of range. */
 size_t nb_workspace_bytes(int64_t n_max);
 
 /* Bind the state.  posm, vel: dev float[n][4], 16-byte aligned, BORROWED and
@@ -124,11 +125,13 @@ int nb_get_launch_info(nb_ctx* ctx, int32_t* out4);
 /* Kernels launched by this ctx since nb_create() (for bench accounting). */
 int64_t nb_launch_count(nb_ctx* ctx);
 
-/* Measurement aid: launch the all-pairs force kernel (row a2/a3 only; its partial
- * sums land in the workspace and touch no state) `reps` times on the ctx stream
- * after one warm-up launch, bracketed by CUDA events on that stream; HOST *ms_avg
- * receives the average duration of one launch.  Synchronises the stream. */
+/* Measurement aids: launch the all-pairs gravity kernel (row a2: Eq. 4 over all N^2 ordered
+ * pairs; nb_time_force_kernel) or the contact pass (row a3: Hilbert keys, sort, gather, Eqs. 5/6;
+ * nb_time_contact_pass, 0 ms when gamma == 0) `reps` times on the ctx stream after one warm-up,
+ * bracketed by CUDA events on that stream; HOST *ms_avg receives the average duration of one
+ * pass.  Their partial sums land in the workspace and touch no state.  Synchronise the stream. */
 int nb_time_force_kernel(nb_ctx* ctx, int reps, float* ms_avg);
+int nb_time_contact_pass(nb_ctx* ctx, int reps, float* ms_avg);
 
 void nb_destroy(nb_ctx* ctx);
 const char* nb_strerror(int status);

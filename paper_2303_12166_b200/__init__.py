@@ -19,7 +19,7 @@ NB_OK, NB_EINVAL, NB_ESTATE, NB_ECUDA, NB_ENOMEM, NB_EARCH = 0, -1, -2, -3, -4, 
 
 EXPORTS = ("nb_create", "nb_workspace_bytes", "nb_set_state", "nb_compute_accel", "nb_step",
            "nb_energy", "nb_get_step", "nb_upload_state", "nb_download_state",
-           "nb_get_launch_info", "nb_launch_count", "nb_time_force_kernel", "nb_destroy", "nb_strerror",
+           "nb_get_launch_info", "nb_launch_count", "nb_time_force_kernel", "nb_time_contact_pass", "nb_destroy", "nb_strerror",
            "nb_last_cuda_error", "nb_roche_lobe_radius", "nb_l1_distance")
 
 
@@ -77,6 +77,8 @@ def lib() -> C.CDLL:
         L.nb_launch_count.argtypes = [vp]
         L.nb_time_force_kernel.restype = C.c_int
         L.nb_time_force_kernel.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
+        L.nb_time_contact_pass.restype = C.c_int
+        L.nb_time_contact_pass.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
         L.nb_destroy.restype = None
         L.nb_destroy.argtypes = [vp]
         L.nb_strerror.restype = C.c_char_p
@@ -185,6 +187,12 @@ def nb_launch_count(ctx: int) -> int:
 def nb_time_force_kernel(ctx: int, reps: int) -> float:
     ms = C.c_float()
     _check(lib().nb_time_force_kernel(ctx, int(reps), C.byref(ms)), "nb_time_force_kernel", ctx)
+    return float(ms.value)
+
+
+def nb_time_contact_pass(ctx: int, reps: int) -> float:
+    ms = C.c_float()
+    _check(lib().nb_time_contact_pass(ctx, int(reps), C.byref(ms)), "nb_time_contact_pass", ctx)
     return float(ms.value)
 
 

@@ -4,6 +4,8 @@
 #include "nb.h"
 #include "nb_kernels.cuh"
 
+#include <cub/device/device_radix_sort.cuh>   // CUDA-toolkit radix sort: orders (Hilbert key, index) pairs only
+
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -20,64 +22,91 @@ constexpr size_t kAlign = 256;
 
 inline size_t align_up(size_t x) { return (x + kAlign - 1) / kAlign * kAlign; }
 
-struct Plan {           // launch configuration of the force kernel for a given n
-    int I = 4;          // elements i per thread
+struct Plan {           // launch configuration of the gravity kernel for a given n
+    int I = 2;          // elements i per thread
     int TJ = 256;       // j tile
     int nib = 0;        // i blocks
     int njt = 0;        // j tiles
     int nsplit = 1;     // j splits P
 };
 
-// Upper bound on nsplit * n over all n <= n_max (partial-sum slab count).
-constexpr int64_t kTargetCtasPerSM = 48;
+constexpr int kCtasPerSM = 8;                      // resident CTAs/SM of nb_gravity_kernel<2, .> (64 registers)
+constexpr int64_t kMaxSplit = 64;
+constexpr int64_t kPartialBudget = (int64_t)128 << 20;   // bytes of split-j partial sums worth keeping in L2
+constexpr int64_t kSortMinN = 8192;                // below this the contact pass takes groups in index order
 
-Plan make_plan(int64_t n, int num_sms)
+// Largest number of j splits allowed for n elements (bounds the partial-sum slabs).
+int64_t max_split(int64_t n)
 {
-    Plan p;
-    if (n >= 16384)      { p.I = 4; p.TJ = 256; }
-    else                 { p.I = 2; p.TJ = 128; }
-#ifdef NB_FORCE_I2
-    p.I = 2; p.TJ = 128;
-#endif
-    const int ib = kThreads * p.I;
-    p.nib = (int)((n + ib - 1) / ib);
-    p.njt = (int)((n + p.TJ - 1) / p.TJ);
-    // enough CTAs that the tail of the last wave is ~1/kTargetCtasPerSM of the run,
-    // but never less than 2 tiles per split
-    const int64_t target = (int64_t)num_sms * kTargetCtasPerSM;
-    int64_t P = (target + p.nib - 1) / p.nib;
-    const int64_t pmax = p.njt >= 2 ? p.njt / 2 : 1;
-    if (P > pmax) P = pmax;
-    if (P < 1) P = 1;
-    p.nsplit = (int)P;
+    int64_t p = kPartialBudget / (16 * n);
+    if (p < 8) p = 8;
+    if (p > kMaxSplit) p = kMaxSplit;
     return p;
 }
 
+// Slabs of n float4: max_split(n) gravity partials + 1 contact slab.  Each term of the bound
+// grows with n, so the value for n_max covers every n <= n_max.
 int64_t partial_elems_bound(int64_t n_max)
 {
-    // nsplit <= target/nib + 1 with nib >= n/512  =>  nsplit*n <= 512*target + n, and
-    // nsplit <= njt/2 with TJ >= 128               =>  nsplit*n <= n^2/256 + n.
-    // Both grow with n, so the bound for n_max covers every n <= n_max.
-    const int64_t target = (int64_t)kNumSMsFallback * 2 * kTargetCtasPerSM;   // margin for > 148 SMs
-    const int64_t b1 = 512 * target + 2 * n_max;
-    const int64_t b2 = n_max * n_max / 256 + 2 * n_max;
-    return b1 < b2 ? b1 : b2;
+    const int64_t a = (kMaxSplit + 1) * n_max;
+    const int64_t b1 = 9 * n_max, b2 = kPartialBudget / 16 + n_max;
+    const int64_t b = b1 > b2 ? b1 : b2;
+    return a < b ? a : b;
+}
+
+// P j-splits give nib*P equal CTAs that run in rounds of `slots` resident CTAs: the cost is
+// rounds x (tiles per split + a per-CTA prologue), with a small term for the ragged end of
+// the last round (CTAs drift apart, so more rounds end more evenly).
+Plan make_plan(int64_t n, int num_sms)
+{
+    Plan p;
+    p.I = 2;
+    p.TJ = n >= 16384 ? 256 : 128;
+    const int ib = kThreads * p.I;
+    p.nib = (int)((n + ib - 1) / ib);
+    p.njt = (int)((n + p.TJ - 1) / p.TJ);
+    const int64_t slots = (int64_t)num_sms * kCtasPerSM;
+    int64_t pmax = p.njt >= 2 ? p.njt / 2 : 1;
+    if (pmax > max_split(n)) pmax = max_split(n);
+    double best = 0.0;
+    for (int64_t P = 1; P <= pmax; ++P) {
+        const int64_t rounds = (p.nib * P + slots - 1) / slots;
+        const int64_t tiles = (p.njt + P - 1) / P;
+        const double cost = (double)rounds * (double)(tiles + 2) * (1.0 + 0.25 / (double)rounds);
+        if (P == 1 || cost < best) { best = cost; p.nsplit = (int)P; }
+    }
+    return p;
 }
 
 struct Layout {
-    size_t off_dev, off_acc, off_part, off_red, total;
+    size_t off_dev, off_acc, off_part, off_red, off_keys, off_vals, off_sorttmp, off_ps, off_vs, off_gbox,
+        off_sbox, off_boxes, total;
+    size_t sorttmp_bytes;
 };
+
+size_t sort_temp_bound(int64_t n_max) { return (size_t)n_max * 16 + ((size_t)8 << 20); }
 
 Layout make_layout(int64_t n_max)
 {
     Layout L;
     size_t o = 0;
+    const size_t ngroups = (size_t)((n_max + kGroup - 1) / kGroup);
+    const size_t nsuper = (ngroups + kSuper - 1) / kSuper;
     L.off_dev = o;  o += align_up(sizeof(DevState));
     L.off_acc = o;  o += align_up((size_t)n_max * sizeof(float4));
     L.off_part = o; o += align_up((size_t)partial_elems_bound(n_max) * sizeof(float4));
     const size_t pot_blocks = (size_t)((n_max + kThreads - 1) / kThreads);
     const size_t red = (size_t)kMomentBlocks * kMomentCols * sizeof(double) + pot_blocks * 2 * sizeof(double);
     L.off_red = o;  o += align_up(red);
+    L.off_keys = o; o += align_up((size_t)n_max * 2 * sizeof(unsigned long long));   // key double buffer
+    L.off_vals = o; o += align_up((size_t)n_max * 2 * sizeof(uint32_t));             // index double buffer
+    L.sorttmp_bytes = sort_temp_bound(n_max);
+    L.off_sorttmp = o; o += align_up(L.sorttmp_bytes);
+    L.off_ps = o;   o += align_up((size_t)n_max * sizeof(float4));
+    L.off_vs = o;   o += align_up((size_t)n_max * sizeof(float4));
+    L.off_gbox = o; o += align_up(ngroups * 2 * sizeof(float4));
+    L.off_sbox = o; o += align_up(nsuper * 2 * sizeof(float4));
+    L.off_boxes = o; o += align_up((size_t)kBoxBlocks * 2 * sizeof(float4));
     L.total = o;
     return L;
 }
@@ -103,6 +132,15 @@ struct nb_ctx {
     float4* acc() const { return reinterpret_cast<float4*>(ws + lay.off_acc); }
     float4* part() const { return reinterpret_cast<float4*>(ws + lay.off_part); }
     double* red() const { return reinterpret_cast<double*>(ws + lay.off_red); }
+    unsigned long long* keys() const { return reinterpret_cast<unsigned long long*>(ws + lay.off_keys); }
+    uint32_t* vals() const { return reinterpret_cast<uint32_t*>(ws + lay.off_vals); }
+    float4* ps() const { return reinterpret_cast<float4*>(ws + lay.off_ps); }
+    float4* vs() const { return reinterpret_cast<float4*>(ws + lay.off_vs); }
+    float4* gbox() const { return reinterpret_cast<float4*>(ws + lay.off_gbox); }
+    float4* sbox() const { return reinterpret_cast<float4*>(ws + lay.off_sbox); }
+    float4* boxes() const { return reinterpret_cast<float4*>(ws + lay.off_boxes); }
+    bool contact_on() const { return prm.gamma > 0.f; }
+    int nslabs() const { return plan.nsplit + (contact_on() ? 1 : 0); }   // slabs nb_reduce_update_kernel sums
 };
 
 #define NB_CUDA(ctx, call)                                   \
@@ -131,32 +169,65 @@ bool params_ok(const nb_params* p)
     return true;
 }
 
-template <int I, int TJ>
-int launch_force_t(nb_ctx* c, const ForceArgs& fa, int grid)
+// Row a2: partial gravitational accelerations of all (i-block, j-split) pairs -> part[0..P-1][n]
+int launch_gravity(nb_ctx* c)
 {
-    if (c->prm.gamma > 0.f)
-        nb_force_kernel<I, TJ, true><<<grid, kThreads, 0, c->stream>>>(fa);
-    else
-        nb_force_kernel<I, TJ, false><<<grid, kThreads, 0, c->stream>>>(fa);
+    GravArgs ga;
+    ga.posm = c->posm; ga.part = c->part();
+    ga.n = (int)c->n; ga.nib = c->plan.nib; ga.nsplit = c->plan.nsplit; ga.njt = c->plan.njt;
+    ga.G = c->prm.G; ga.eps = c->prm.eps;
+    const int grid = c->plan.nib * c->plan.nsplit;
+    if (c->plan.TJ == 256) nb_gravity_kernel<2, 256><<<grid, kThreads, 0, c->stream>>>(ga);
+    else                   nb_gravity_kernel<2, 128><<<grid, kThreads, 0, c->stream>>>(ga);
     c->launches++;
     NB_CUDA(c, cudaGetLastError());
     return NB_OK;
 }
 
-// Row a2/a3: partial accelerations of all (i-block, j-split) pairs -> part[P][n]
+// Row a3: contact accelerations (Eqs. 5/6) of the pairs with r < R_i + R_j -> part[P][n]
+int launch_contact(nb_ctx* c)
+{
+    const int n = (int)c->n;
+    const uint32_t* perm = nullptr;
+    if (c->n >= kSortMinN) {
+        nb_bbox_kernel<<<kBoxBlocks, 256, 0, c->stream>>>(c->posm, n, c->boxes());
+        c->launches++;
+        nb_keys_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->posm, n, c->boxes(), c->keys(), c->vals());
+        c->launches++;
+        NB_CUDA(c, cudaGetLastError());
+        cub::DoubleBuffer<unsigned long long> dk(c->keys(), c->keys() + c->n_max);
+        cub::DoubleBuffer<uint32_t> dv(c->vals(), c->vals() + c->n_max);
+        size_t tmp = c->lay.sorttmp_bytes;
+        NB_CUDA(c, cub::DeviceRadixSort::SortPairs(c->ws + c->lay.off_sorttmp, tmp, dk, dv, n, 0, 3 * kKeyBits, c->stream));
+        c->launches += 1;                              // counted as one (library) launch
+        perm = dv.Current();
+    }
+    const int ngroups = (n + kGroup - 1) / kGroup;
+    const int nsuper = (ngroups + kSuper - 1) / kSuper;
+    nb_gather_kernel<<<nsuper, kGroup * kSuper, 0, c->stream>>>(c->posm, c->vel, perm, n, c->dev(), c->ps(), c->vs(),
+                                                               c->gbox(), c->sbox());
+    c->launches++;
+    ContactArgs ca;
+    ca.ps = c->ps(); ca.vs = c->vs(); ca.perm = perm; ca.gbox = c->gbox(); ca.sbox = c->sbox();
+    ca.out = c->part() + (size_t)c->plan.nsplit * c->n;
+    ca.n = n; ca.ngroups = ngroups; ca.nsuper = nsuper;
+    ca.gamma = c->prm.gamma; ca.gamma_beta = c->prm.gamma * c->prm.beta;
+    ca.v_dead = c->prm.v_dead; ca.lens_mode = c->prm.lens_mode;
+    nb_contact_kernel<<<(ngroups * 32 + kThreads - 1) / kThreads, kThreads, 0, c->stream>>>(ca);
+    c->launches++;
+    NB_CUDA(c, cudaGetLastError());
+    return NB_OK;
+}
+
+// Rows a2 + a3: every slab nb_reduce_update_kernel sums for a(x).  The contact pass goes first:
+// it is short, and the gravity kernel's CTAs then fill the machine behind it.
 int launch_force(nb_ctx* c)
 {
-    ForceArgs fa;
-    fa.posm = c->posm; fa.vel = c->vel; fa.dev = c->dev(); fa.part = c->part();
-    fa.n = (int)c->n; fa.n1 = c->n1; fa.nib = c->plan.nib; fa.nsplit = c->plan.nsplit; fa.njt = c->plan.njt;
-    fa.G = c->prm.G; fa.eps = c->prm.eps;
-    fa.gamma = c->prm.gamma; fa.gamma_beta = c->prm.gamma * c->prm.beta;
-    fa.v_dead = c->prm.v_dead; fa.lens_mode = c->prm.lens_mode;
-    const int grid = c->plan.nib * c->plan.nsplit;
-    switch (c->plan.I) {
-        case 4: return launch_force_t<4, 256>(c, fa, grid);
-        default: return launch_force_t<2, 128>(c, fa, grid);
+    if (c->contact_on()) {
+        const int rc = launch_contact(c);
+        if (rc) return rc;
     }
+    return launch_gravity(c);
 }
 
 // Rows a4+a6+a5: reduce `nsrc` slabs of `src`, optionally store a, kick, drift, advance.
@@ -178,7 +249,7 @@ int ensure_acc(nb_ctx* c)
     if (c->have_acc) return NB_OK;
     int rc = launch_force(c);
     if (rc) return rc;
-    rc = launch_update(c, c->part(), c->plan.nsplit, c->acc(), 0.f, 0.f, 0);
+    rc = launch_update(c, c->part(), c->nslabs(), c->acc(), 0.f, 0.f, 0);
     if (rc) return rc;
     c->have_acc = true;
     return NB_OK;
@@ -226,6 +297,16 @@ int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream
     c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     c->num_sms = sms > 0 ? sms : kNumSMsFallback;
     c->lay = make_layout(n_max);
+    {   // the radix sort's scratch must fit the slice the layout reserves for it
+        size_t need = 0;
+        cub::DoubleBuffer<unsigned long long> dk(nullptr, nullptr);
+        cub::DoubleBuffer<uint32_t> dv(nullptr, nullptr);
+        if (cub::DeviceRadixSort::SortPairs(nullptr, need, dk, dv, (int)n_max, 0, 3 * kKeyBits, c->stream) != cudaSuccess ||
+            need > c->lay.sorttmp_bytes) {
+            delete c;
+            return NB_ENOMEM;
+        }
+    }
     *out = c;
     return NB_OK;
 }
@@ -266,7 +347,7 @@ int nb_set_state(nb_ctx* c, int64_t n, float* posm, float* vel, const int32_t* s
     c->posm = reinterpret_cast<float4*>(posm);
     c->vel = reinterpret_cast<float4*>(vel);
     c->plan = make_plan(n, c->num_sms);
-    if ((int64_t)c->plan.nsplit * n > partial_elems_bound(c->n_max)) return NB_ENOMEM;
+    if ((int64_t)(c->plan.nsplit + 1) * n > partial_elems_bound(c->n_max)) return NB_ENOMEM;
     c->have_state = true;
     return NB_OK;
 }
@@ -277,7 +358,7 @@ int nb_compute_accel(nb_ctx* c, float* acc)
     if (!c->have_state) return NB_ESTATE;
     int rc = launch_force(c);
     if (rc) return rc;
-    rc = launch_update(c, c->part(), c->plan.nsplit, reinterpret_cast<float4*>(acc), 0.f, 0.f, 0);
+    rc = launch_update(c, c->part(), c->nslabs(), reinterpret_cast<float4*>(acc), 0.f, 0.f, 0);
     if (rc) return rc;
     if (reinterpret_cast<float4*>(acc) != c->acc()) {
         NB_CUDA(c, cudaMemcpyAsync(c->acc(), acc, (size_t)c->n * sizeof(float4), cudaMemcpyDeviceToDevice,
@@ -302,9 +383,9 @@ int nb_step(nb_ctx* c, int nsteps)
         rc = launch_force(c);                                  // a(x_{n+s}) with v_{n+s-1/2}
         if (rc) return rc;
         if (s < nsteps)   // two half kicks merged: v += dt a ; x += dt v ; advance
-            rc = launch_update(c, c->part(), c->plan.nsplit, nullptr, dt, dt, 1);
+            rc = launch_update(c, c->part(), c->nslabs(), nullptr, dt, dt, 1);
         else              // closing half kick; cache a(x_{n+nsteps})
-            rc = launch_update(c, c->part(), c->plan.nsplit, c->acc(), 0.5f * dt, 0.f, 0);
+            rc = launch_update(c, c->part(), c->nslabs(), c->acc(), 0.5f * dt, 0.f, 0);
         if (rc) return rc;
     }
     c->have_acc = true;
@@ -409,17 +490,18 @@ int nb_get_launch_info(nb_ctx* c, int32_t* out4)
 
 int64_t nb_launch_count(nb_ctx* c) { return c ? c->launches : 0; }
 
-int nb_time_force_kernel(nb_ctx* c, int reps, float* ms_avg)
+namespace {
+int time_launches(nb_ctx* c, int reps, float* ms_avg, int (*launch)(nb_ctx*))
 {
     if (!c || !ms_avg || reps < 1) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
     cudaEvent_t e0, e1;
     NB_CUDA(c, cudaEventCreate(&e0));
     NB_CUDA(c, cudaEventCreate(&e1));
-    int rc = launch_force(c);                                  // warm-up, untimed
+    int rc = launch(c);                                        // warm-up, untimed
     if (rc == NB_OK) {
         cudaEventRecord(e0, c->stream);
-        for (int r = 0; r < reps && rc == NB_OK; ++r) rc = launch_force(c);
+        for (int r = 0; r < reps && rc == NB_OK; ++r) rc = launch(c);
         cudaEventRecord(e1, c->stream);
     }
     cudaError_t e = cudaEventSynchronize(e1);
@@ -431,6 +513,18 @@ int nb_time_force_kernel(nb_ctx* c, int reps, float* ms_avg)
     if (e != cudaSuccess) { c->last_cuda = (int)e; return NB_ECUDA; }
     *ms_avg = ms / (float)reps;
     return NB_OK;
+}
+}  // namespace
+
+int nb_time_force_kernel(nb_ctx* c, int reps, float* ms_avg)
+{
+    return time_launches(c, reps, ms_avg, launch_gravity);
+}
+
+int nb_time_contact_pass(nb_ctx* c, int reps, float* ms_avg)
+{
+    if (c && !c->contact_on()) { if (ms_avg) *ms_avg = 0.f; return c->have_state ? NB_OK : NB_ESTATE; }
+    return time_launches(c, reps, ms_avg, launch_contact);
 }
 
 double nb_roche_lobe_radius(double mass_ratio, double k)

@@ -1,16 +1,18 @@
 // nb_kernels.cuh -- sm_100a kernels of the all-pairs binary-star element model.
 //
 // Hot path:
-//   a2/a3  nb_force_kernel        all-pairs Eq. 4 gravity with the contact terms of
-//                                 Eqs. 5/6 on a warp-voted slow path
-//   a4/a6  nb_reduce_update_kernel split-j partial-sum reduction fused with the
-//                                 leapfrog kick/drift and the expanding-star rule
-//                                 (PAPER.md:89)
+//   a2     nb_gravity_kernel        all-pairs Eq. 4 gravity, every ordered pair
+//   a3     nb_contact_kernel        contact terms of Eqs. 5/6 for exactly the
+//                                   pairs with r < R_i + R_j, found through Hilbert-ordered groups
+//                                   of 32 elements and their bounding boxes
+//          (nb_bbox_kernel, nb_keys_kernel, [radix sort], nb_gather_kernel build that order)
+//   a4/a6  nb_reduce_update_kernel  partial-sum reduction fused with the leapfrog kick/drift and
+//                                   the expanding-star rule
 //   a7     nb_potential_kernel / nb_moments_kernel   diagnostics for nb_energy
 //
-// The force kernel is bound by the plain FP32 ALUs (FMA pipe, with the XU pipe close
-// behind): per interaction 13 FP32 operations issued as packed FFMA2/FADD2/FMUL2,
-// one MUFU.RSQ and half a MUFU.RCP.  Not a dense contraction: no tensor cores.
+// The gravity kernel is bound by the plain FP32 ALUs (FMA pipe; register-file read bandwidth
+// and the XU pipe close behind): per interaction 13.5 FP32 operations issued as packed
+// FFMA2/FADD2/FMUL2, one MUFU.RSQ and half a MUFU.RCP.  Not a dense contraction: no tensor cores.
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -18,7 +20,8 @@
 namespace nb {
 
 constexpr int kThreads = 128;          // 4 warps: one per SM sub-partition
-constexpr float kTinyR2 = 1.0e-20f;    // added to r^2: keeps the self pair (d = 0) finite, even for eps = 0
+constexpr float kTinyR2 = 1.0e-18f;    // added to r^2: keeps the self pair (d = 0) finite even for eps = 0,
+                                       // and t0*t1 of a Montgomery pair above the fp32 normal range
 constexpr float kFarAway = 1.0e10f;    // padding elements sit here with zero mass
 
 // Device-resident mutable state (head of the workspace); updated on the device so
@@ -31,18 +34,6 @@ struct DevState {
     double R_start[2], R_end[2];
     long long n_ramp;
     long long pad_[2];
-};
-
-struct ForceArgs {
-    const float4* __restrict__ posm;   // [n] x,y,z,m
-    const float4* __restrict__ vel;    // [n] vx,vy,vz,-
-    const DevState* __restrict__ dev;
-    float4* __restrict__ part;         // [nsplit][n] partial accelerations
-    int n, n1, nib, nsplit, njt;
-    float G, eps;
-    float gamma, gamma_beta;           // Eq. 5 / Eq. 6 strengths
-    float v_dead;
-    int lens_mode;
 };
 
 __device__ __forceinline__ float rsqrt_approx(float x) {
@@ -77,75 +68,79 @@ __device__ __forceinline__ float star_radius(int idx, int n1, float R0, float R1
     return idx < n1 ? R0 : R1;
 }
 
-// Slow path: the contact term of one (i, j) pair, Eqs. 5/6, added
-// to the fp64 accumulators of i: a_i -= g pi V(r; R_ij) / m_i * d/r if r < R_i + R_j.
-// d is the fp32 difference the fast path used (exact for near pairs); everything
-// else is evaluated in double (B200 has full-rate-class fp64; ~5/N of all pairs come
-// here, and h = 2R - r cancels badly in fp32 near first contact).
-// lens_mode 0: pi V = pi (D - r)^2 (2D + r) / 12 with D = 2 R_ij (factored displaced
-// volume, A1); lens_mode 1: the polynomial as printed (PAPER.md:80), last term r^2/12.
-__device__ __forceinline__ void contact_term(const ForceArgs& a, int i, int j, float dxf, float dyf, float dzf,
-                                             float R0, float R1, double& ax, double& ay, double& az)
-{
-    if (i >= a.n || j >= a.n || i == j) return;
-    const double dx = dxf, dy = dyf, dz = dzf;
-    const double r2 = dx * dx + dy * dy + dz * dz;
-    const double D = (double)star_radius(i, a.n1, R0, R1) + (double)star_radius(j, a.n1, R0, R1);  // 2 R_ij (A2)
-    if (!(r2 < D * D) || r2 == 0.0) return;                // not in contact / coincident (A3)
-    const double r = sqrt(r2);
-    const double rinv = 1.0 / r;
-    const float4 vi = a.vel[i], vj = a.vel[j];
-    const double rdot = (dx * ((double)vj.x - (double)vi.x) + dy * ((double)vj.y - (double)vi.y)
-                       + dz * ((double)vj.z - (double)vi.z)) * rinv;
-    const double g = (rdot < -(double)a.v_dead) ? (double)a.gamma : (double)a.gamma_beta;  // Eq. 5 : Eq. 6 (A5)
-    const double kPi = 3.14159265358979323846;
-    double piV;
-    if (a.lens_mode == 0) {
-        const double h = D - r;
-        piV = (kPi / 12.0) * h * h * (2.0 * D + r);
-    } else {
-        const double R = 0.5 * D;
-        piV = kPi * ((4.0 / 3.0) * R * R * R - R * R * r + r * r / 12.0);
-    }
-    const double c = -g * piV / (double)a.posm[i].w * rinv;
-    ax += c * dx; ay += c * dy; az += c * dz;
-}
-
-// All-pairs acceleration, one CTA per (i-block, j-split).
+// ---------------------------------------------------------------------------
+// Row a2: all-pairs gravity, Eq. 4, one CTA per (i-block, j-split).
+//
+//   a_i += G m_j / (r + eps)^2 * d/r,   d = x_j - x_i,  every j (the self pair has d = 0)
 //
 // Each thread keeps I (even) elements i in registers as I/2 packed pairs; the CTA
-// streams its j range through shared memory in tiles of TJ elements
-// (double-buffered, one barrier per tile); every LDS.128 of (x_j, y_j, z_j, G m_j)
-// is a warp broadcast reused for I pairs.  Per pair of interactions (one packed
-// lane pair) the loop issues 13 packed FP32 instructions (FADD2 x3, FFMA2 x7,
-// FMUL2 x3), 2 MUFU.RSQ, and ONE MUFU.RCP shared by the two lanes through a
-// two-term Montgomery inversion (3 scalar FMUL): 1/t0 = t1/(t0 t1), 1/t1 = t0/(t0 t1),
-// with t = (r+eps)^2 >= eps^2 so the product cannot underflow.  That moves the
-// bound from the XU pipe (16 lanes/clk/SM) to the FMA pipe.
-// Per-tile fp32 partial sums are flushed into fp64 accumulators (short chains).
-// Contacts (CONTACT): the minimum r^2 over a group of kGroupJ elements j (FMNMX3 on
-// the ALU pipe) is tested once per group against the tile's (R_i+R_j)^2 bound;
-// candidate groups go to a small per-thread queue in shared memory and are
-// resolved after the tile's loop by contact_term().
-constexpr int kQueueDepth = 16;
-#ifndef NB_MINB4
-#define NB_MINB4 4      // resident CTAs/SM the I=4 kernel is compiled for (register cap 65536/(128*NB_MINB4))
-#endif
-#ifndef NB_UNROLL
-#define NB_UNROLL 4
-#endif
-constexpr int kGroupJ = NB_UNROLL;    // elements j per unrolled group = granularity of the contact test
+// streams its j range through shared memory in tiles of TJ elements (double-buffered,
+// one barrier per tile); every LDS.128 of (x_j, y_j, z_j, G m_j) is a warp broadcast.
+// Per packed lane pair and TWO elements j the loop issues
+//     FADD2 x6 (d), FFMA2 x6 (r^2), MUFU.RSQ x4 (y = 1/r), FFMA2 x2 (s = r^2 y + eps),
+//     FMUL2 x2 (t = s^2), FMUL2 (P = t0 t1), MUFU.RCP x2 (1/P), FMUL2 x2 (k0 = t1 y0, k1 = t0 y1),
+//     FMUL2 x2 (c = k/P = y/t), FFMA2 x6 (a += c d)
+// i.e. 13.5 packed FP32 instructions and 1.5 MUFU per interaction: the reciprocal of
+// (r+eps)^2 is shared by the two j of a lane (Montgomery's trick: 1/t0 = t1/(t0 t1)), entirely
+// in packed form.  t >= max(eps^2, kTinyR2) so the product cannot underflow; a padding element
+// (1e10 away) overflows P to +inf -> 1/P = 0 -> contributes exactly 0.
+// Tiles whose elements all have the same mass (the paper's stars are made of equal-mass
+// elements) skip the per-pair multiply by G m_j: the tile's fp32 sums are
+// scaled once when they are flushed into the fp64 accumulators.  Other tiles multiply k by
+// G m_j (one more FMUL2 per lane pair and j).
+struct GravArgs {
+    const float4* __restrict__ posm;   // [n] x,y,z,m
+    float4* __restrict__ part;         // [nsplit][n] partial accelerations
+    int n, nib, nsplit, njt;
+    float G, eps;
+};
 
-template <int I, int TJ, bool CONTACT>
-__global__ void __launch_bounds__(kThreads, (I >= 4 ? NB_MINB4 : 6))
-nb_force_kernel(const __grid_constant__ ForceArgs a)
+constexpr int kGroupJ = 4;             // elements j per unrolled group (two Montgomery pairs)
+
+template <int H, bool UNI>
+__device__ __forceinline__ void gravity_group(const float4* __restrict__ s,
+                                              const f32x2 (&nxi)[H], const f32x2 (&nyi)[H], const f32x2 (&nzi)[H],
+                                              f32x2 eps2, f32x2 (&ax)[H], f32x2 (&ay)[H], f32x2 (&az)[H])
 {
-    static_assert(I % 2 == 0 && TJ % kThreads == 0 && TJ % kGroupJ == 0 && TJ / kGroupJ <= 256,
-                  "packed pairs; whole groups; group index fits a byte");
+    const f32x2 tiny2 = pk2(kTinyR2, kTinyR2);
+#pragma unroll
+    for (int u = 0; u < kGroupJ; u += 2) {
+        const float4 p0 = s[u], p1 = s[u + 1];                     // LDS.128 broadcasts
+        const f32x2 x0 = pk2(p0.x, p0.x), y0 = pk2(p0.y, p0.y), z0 = pk2(p0.z, p0.z);
+        const f32x2 x1 = pk2(p1.x, p1.x), y1 = pk2(p1.y, p1.y), z1 = pk2(p1.z, p1.z);
+#pragma unroll
+        for (int h = 0; h < H; ++h) {
+            const f32x2 dx0 = add2(x0, nxi[h]), dy0 = add2(y0, nyi[h]), dz0 = add2(z0, nzi[h]);
+            const f32x2 dx1 = add2(x1, nxi[h]), dy1 = add2(y1, nyi[h]), dz1 = add2(z1, nzi[h]);
+            f32x2 r20 = fma2(dx0, dx0, tiny2); r20 = fma2(dy0, dy0, r20); r20 = fma2(dz0, dz0, r20);
+            f32x2 r21 = fma2(dx1, dx1, tiny2); r21 = fma2(dy1, dy1, r21); r21 = fma2(dz1, dz1, r21);
+            float a0, b0, a1, b1;
+            unpk2(r20, a0, b0); unpk2(r21, a1, b1);
+            const f32x2 ri0 = pk2(rsqrt_approx(a0), rsqrt_approx(b0));     // 1/r
+            const f32x2 ri1 = pk2(rsqrt_approx(a1), rsqrt_approx(b1));
+            const f32x2 s0 = fma2(r20, ri0, eps2), s1 = fma2(r21, ri1, eps2);   // r + eps
+            const f32x2 t0 = mul2(s0, s0), t1 = mul2(s1, s1);                   // (r + eps)^2
+            const f32x2 P = mul2(t0, t1);
+            float pl, ph;
+            unpk2(P, pl, ph);
+            const f32x2 iP = pk2(rcp_approx(pl), rcp_approx(ph));              // one RCP per two interactions
+            f32x2 k0 = mul2(t1, ri0), k1 = mul2(t0, ri1);
+            if (!UNI) { k0 = mul2(k0, pk2(p0.w, p0.w)); k1 = mul2(k1, pk2(p1.w, p1.w)); }   // G m_j
+            const f32x2 c0 = mul2(iP, k0), c1 = mul2(iP, k1);                  // [G m_j]/(r (r+eps)^2)  Eq. 4
+            ax[h] = fma2(c0, dx0, ax[h]); ay[h] = fma2(c0, dy0, ay[h]); az[h] = fma2(c0, dz0, az[h]);
+            ax[h] = fma2(c1, dx1, ax[h]); ay[h] = fma2(c1, dy1, ay[h]); az[h] = fma2(c1, dz1, az[h]);
+        }
+    }
+}
+
+template <int I, int TJ>
+__global__ void __launch_bounds__(kThreads, (I == 2 ? 8 : 4))
+nb_gravity_kernel(const __grid_constant__ GravArgs a)
+{
+    static_assert(I % 2 == 0 && TJ % kThreads == 0 && TJ % kGroupJ == 0, "packed pairs; whole groups");
     constexpr int H = I / 2;                        // packed pairs per thread
     constexpr int LPT = TJ / kThreads;              // tile loads per thread
     __shared__ float4 sj[2][TJ];
-    __shared__ unsigned char queue[CONTACT ? kQueueDepth * kThreads : 1];
 
     const int tid = threadIdx.x;
     const int ib = blockIdx.x % a.nib;
@@ -169,7 +164,6 @@ nb_force_kernel(const __grid_constant__ ForceArgs a)
         nxi[h] = pk2(px[0], px[1]); nyi[h] = pk2(py[0], py[1]); nzi[h] = pk2(pz[0], pz[1]);
     }
 
-    const float R0 = a.dev->R[0], R1 = a.dev->R[1];
     const int t0 = (int)(((long long)sp * a.njt) / a.nsplit);
     const int t1 = (int)(((long long)(sp + 1) * a.njt) / a.nsplit);
 
@@ -177,26 +171,24 @@ nb_force_kernel(const __grid_constant__ ForceArgs a)
 #pragma unroll
     for (int k = 0; k < I; ++k) accx[k] = accy[k] = accz[k] = 0.0;
 
-    // contact bound of this thread's elements: (max R_i + max R_j)^2 per tile
-    float Ri_max = 0.f;
-    if (CONTACT) {
-        const int ilast = min(ibase + (I - 1) * kThreads, a.n - 1);
-        Ri_max = (ibase < a.n1 && ilast >= a.n1) ? fmaxf(R0, R1)
-                                                 : star_radius(min(ibase, a.n - 1), a.n1, R0, R1);
-    }
-
     float4 pre[LPT];
+    bool my_uni = false;                             // this thread's share of the tile has one mass
     auto load_tile = [&](int t) {
+        const float mref = a.posm[min(t * TJ, a.n - 1)].w;
+        bool u = true;
 #pragma unroll
         for (int l = 0; l < LPT; ++l) {
             const int j = t * TJ + l * kThreads + tid;
             if (j < a.n) {
                 pre[l] = a.posm[j];
+                u = u && (pre[l].w == mref);
                 pre[l].w *= a.G;                                   // fold G into m_j
             } else {
                 pre[l] = make_float4(kFarAway, kFarAway, kFarAway, 0.f);
+                u = false;
             }
         }
+        my_uni = u;
     };
     auto store_tile = [&](int buf) {
 #pragma unroll
@@ -204,9 +196,8 @@ nb_force_kernel(const __grid_constant__ ForceArgs a)
     };
 
     if (t0 < t1) { load_tile(t0); store_tile(0); }
-    __syncthreads();
+    int uni = __syncthreads_and(my_uni ? 1 : 0);
 
-    const f32x2 tiny2 = pk2(kTinyR2, kTinyR2);
     const f32x2 eps2 = pk2(a.eps, a.eps);
 
     for (int t = t0; t < t1; ++t) {
@@ -217,94 +208,30 @@ nb_force_kernel(const __grid_constant__ ForceArgs a)
 #pragma unroll
         for (int h = 0; h < H; ++h) ax[h] = ay[h] = az[h] = pk2(0.f, 0.f);
 
-        float rc2 = 0.f;
-        if (CONTACT) {
-            const int jb = t * TJ, je = min(jb + TJ, a.n) - 1;
-            const float Rj_max = (jb < a.n1 && je >= a.n1) ? fmaxf(R0, R1)
-                                                           : star_radius(jb, a.n1, R0, R1);
-            const float D = Ri_max + Rj_max;
-            rc2 = D * D;
-        }
-        int qn = 0;                                  // candidate groups pushed in this tile
-
         const float4* __restrict__ s = sj[buf];
+        double scale = 1.0;
+        if (uni) {
 #pragma unroll 1
-        for (int jg = 0; jg < TJ; jg += kGroupJ) {
-            float rmin = 3.0e38f;
-#pragma unroll
-            for (int u_ = 0; u_ < kGroupJ; ++u_) {
-                const float4 pj = s[jg + u_];            // LDS.128 broadcast
-                const f32x2 xj = pk2(pj.x, pj.x), yj = pk2(pj.y, pj.y), zj = pk2(pj.z, pj.z);
-#pragma unroll
-                for (int h = 0; h < H; ++h) {
-                    const f32x2 dx = add2(xj, nxi[h]);
-                    const f32x2 dy = add2(yj, nyi[h]);
-                    const f32x2 dz = add2(zj, nzi[h]);
-                    f32x2 r2 = fma2(dx, dx, tiny2);
-                    r2 = fma2(dy, dy, r2);
-                    r2 = fma2(dz, dz, r2);
-                    float r2l, r2h;
-                    unpk2(r2, r2l, r2h);
-                    const f32x2 y = pk2(rsqrt_approx(r2l), rsqrt_approx(r2h));   // 1/r
-                    const f32x2 sft = fma2(r2, y, eps2);                           // r + eps
-                    const f32x2 tt = mul2(sft, sft);                               // (r+eps)^2
-                    float tl, th;
-                    unpk2(tt, tl, th);
-                    const float ipm = rcp_approx(tl * th) * pj.w;                  // one RCP for both lanes
-                    const f32x2 um = pk2(ipm * th, ipm * tl);                      // G m_j/(r+eps)^2
-                    const f32x2 c = mul2(um, y);                                   // G m_j/(r (r+eps)^2)  Eq. 4
-                    ax[h] = fma2(c, dx, ax[h]);
-                    ay[h] = fma2(c, dy, ay[h]);
-                    az[h] = fma2(c, dz, az[h]);
-                    if (CONTACT) rmin = fminf(rmin, fminf(r2l, r2h));              // FMNMX3
-                }
-            }
-            if (CONTACT) {
-                if (rmin < rc2) {                    // rare: one branch per kGroupJ elements j
-                    queue[(qn & (kQueueDepth - 1)) * kThreads + tid] = (unsigned char)(jg / kGroupJ);
-                    ++qn;
-                }
-            }
+            for (int jg = 0; jg < TJ; jg += kGroupJ)
+                gravity_group<H, true>(s + jg, nxi, nyi, nzi, eps2, ax, ay, az);
+            scale = (double)s[0].w;                  // G m of the whole tile
+        } else {
+#pragma unroll 1
+            for (int jg = 0; jg < TJ; jg += kGroupJ)
+                gravity_group<H, false>(s + jg, nxi, nyi, nzi, eps2, ax, ay, az);
         }
 
+        // flush the tile's fp32 sums into the fp64 accumulators (short fp32 chains)
 #pragma unroll
         for (int h = 0; h < H; ++h) {
             float l, hgh;
-            unpk2(ax[h], l, hgh); accx[2 * h] += (double)l; accx[2 * h + 1] += (double)hgh;
-            unpk2(ay[h], l, hgh); accy[2 * h] += (double)l; accy[2 * h + 1] += (double)hgh;
-            unpk2(az[h], l, hgh); accz[2 * h] += (double)l; accz[2 * h + 1] += (double)hgh;
-        }
-
-        if (CONTACT && qn > 0) {
-            // Resolve this thread's candidate groups (the whole tile if the queue overflowed).
-            const bool all = qn > kQueueDepth;
-            const int cnt = all ? TJ / kGroupJ : qn;
-#pragma unroll 1
-            for (int q = 0; q < cnt; ++q) {
-                const int jg = kGroupJ * (all ? q : (int)queue[q * kThreads + tid]);
-#pragma unroll 1
-                for (int jj = jg; jj < jg + kGroupJ; ++jj) {
-                    const float4 pj = s[jj];
-                    const int j = t * TJ + jj;
-#pragma unroll
-                    for (int h = 0; h < H; ++h) {
-                        float xl, xh, yl, yh, zl, zh;
-                        unpk2(nxi[h], xl, xh); unpk2(nyi[h], yl, yh); unpk2(nzi[h], zl, zh);
-                        const float dxl = pj.x + xl, dyl = pj.y + yl, dzl = pj.z + zl;
-                        const float dxh = pj.x + xh, dyh = pj.y + yh, dzh = pj.z + zh;
-                        if (fmaf(dzl, dzl, fmaf(dyl, dyl, dxl * dxl)) < rc2)
-                            contact_term(a, ibase + (2 * h) * kThreads, j, dxl, dyl, dzl, R0, R1,
-                                         accx[2 * h], accy[2 * h], accz[2 * h]);
-                        if (fmaf(dzh, dzh, fmaf(dyh, dyh, dxh * dxh)) < rc2)
-                            contact_term(a, ibase + (2 * h + 1) * kThreads, j, dxh, dyh, dzh, R0, R1,
-                                         accx[2 * h + 1], accy[2 * h + 1], accz[2 * h + 1]);
-                    }
-                }
-            }
+            unpk2(ax[h], l, hgh); accx[2 * h] += scale * (double)l; accx[2 * h + 1] += scale * (double)hgh;
+            unpk2(ay[h], l, hgh); accy[2 * h] += scale * (double)l; accy[2 * h + 1] += scale * (double)hgh;
+            unpk2(az[h], l, hgh); accz[2 * h] += scale * (double)l; accz[2 * h + 1] += scale * (double)hgh;
         }
 
         if (t + 1 < t1) store_tile(buf ^ 1);
-        __syncthreads();
+        uni = __syncthreads_and(my_uni ? 1 : 0);
     }
 
     float4* __restrict__ out = a.part + (size_t)sp * a.n;
@@ -312,6 +239,319 @@ nb_force_kernel(const __grid_constant__ ForceArgs a)
     for (int k = 0; k < I; ++k) {
         const int i = ibase + k * kThreads;
         if (i < a.n) out[i] = make_float4((float)accx[k], (float)accy[k], (float)accz[k], 0.f);
+    }
+}
+
+// ---------------------------------------------------------------------------
+// Row a3: contact repulsion, Eqs. 5/6, for exactly the pairs with
+// r < R_i + R_j.  These are ~5 pairs per element out of N, so they are found by a spatial
+// search instead of a test inside the N^2 loop:
+//   nb_bbox_kernel    bounding box of all elements (block partials, no atomics)
+//   nb_keys_kernel    48-bit Hilbert-curve key of every element inside that box
+//   [radix sort of (key, index) -> perm; host side, nb_api.cu]
+//   nb_gather_kernel  elements in Hilbert order: ps = (x,y,z,R_star), vs = (vx,vy,vz,m);
+//                     bounding box + largest radius of every group of 32 and of every
+//                     super-group of 32 groups
+//   nb_contact_kernel one warp per group of 32 elements i (one per lane): scan the super-group
+//                     boxes, then the group boxes of the near super-groups (box against box), then
+//                     each lane's point against the box of every candidate group, then every j of
+//                     the groups that survive; a pair in contact is evaluated in fp64.
+// The box tests are conservative (a pair in contact is never skipped); which pairs ARE in
+// contact is decided by the fp64 test r < R_i + R_j alone, so the result does not depend on
+// the order.  For small n the sort is skipped (perm == nullptr: groups in index order).
+constexpr int kBoxBlocks = 128;       // partial boxes of nb_bbox_kernel
+constexpr int kGroup = 32;            // elements per group (one warp)
+constexpr int kSuper = 32;            // groups per super-group (one 1024-thread block of the gather)
+
+__device__ __forceinline__ float warp_min(float v) {
+    for (int o = 16; o > 0; o >>= 1) v = fminf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ float warp_max(float v) {
+    for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+
+// boxes[2b] = (lo.xyz, 0), boxes[2b+1] = (hi.xyz, 0) of block b's grid-stride share.
+__global__ void __launch_bounds__(256)
+nb_bbox_kernel(const float4* __restrict__ posm, int n, float4* __restrict__ boxes)
+{
+    __shared__ float sh[6][8];
+    float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const float4 p = posm[i];
+        lo[0] = fminf(lo[0], p.x); lo[1] = fminf(lo[1], p.y); lo[2] = fminf(lo[2], p.z);
+        hi[0] = fmaxf(hi[0], p.x); hi[1] = fmaxf(hi[1], p.y); hi[2] = fmaxf(hi[2], p.z);
+    }
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    for (int c = 0; c < 3; ++c) {
+        const float a = warp_min(lo[c]), b = warp_max(hi[c]);
+        if (l == 0) { sh[c][w] = a; sh[3 + c][w] = b; }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int c = 0; c < 3; ++c)
+            for (int k = 1; k < 8; ++k) { sh[c][0] = fminf(sh[c][0], sh[c][k]); sh[3 + c][0] = fmaxf(sh[3 + c][0], sh[3 + c][k]); }
+        boxes[2 * blockIdx.x] = make_float4(sh[0][0], sh[1][0], sh[2][0], 0.f);
+        boxes[2 * blockIdx.x + 1] = make_float4(sh[3][0], sh[4][0], sh[5][0], 0.f);
+    }
+}
+
+// Spread the low 16 bits of v to every third bit.
+__device__ __forceinline__ unsigned long long spread3(unsigned long long v) {
+    v &= 0xffffull;
+    v = (v | (v << 16)) & 0x0000ff0000ffull;
+    v = (v | (v << 8))  & 0x00f00f00f00full;
+    v = (v | (v << 4))  & 0x0c30c30c30c3ull;
+    v = (v | (v << 2))  & 0x249249249249ull;
+    return v;
+}
+
+constexpr int kKeyBits = 16;          // bits per axis; keys have 3*kKeyBits = 48 significant bits
+
+// Index of the cell (qx, qy, qz) along the 3-D Hilbert curve of order kKeyBits (Skilling's
+// axes-to-transpose transform, then bit interleave).  Unlike the Z-order curve it has no
+// jumps, so 32 consecutive elements always form a compact group.
+__device__ __forceinline__ unsigned long long hilbert_key(uint32_t qx, uint32_t qy, uint32_t qz) {
+    uint32_t X[3] = {qx, qy, qz};
+    for (uint32_t Q = 1u << (kKeyBits - 1); Q > 1; Q >>= 1) {
+        const uint32_t P = Q - 1;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            if (X[i] & Q) X[0] ^= P;
+            else { const uint32_t t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
+        }
+    }
+    X[1] ^= X[0]; X[2] ^= X[1];
+    uint32_t t = 0;
+    for (uint32_t Q = 1u << (kKeyBits - 1); Q > 1; Q >>= 1)
+        if (X[2] & Q) t ^= Q - 1;
+    X[0] ^= t; X[1] ^= t; X[2] ^= t;
+    return (spread3(X[0]) << 2) | (spread3(X[1]) << 1) | spread3(X[2]);
+}
+
+__global__ void __launch_bounds__(256)
+nb_keys_kernel(const float4* __restrict__ posm, int n, const float4* __restrict__ boxes,
+               unsigned long long* __restrict__ keys, uint32_t* __restrict__ vals)
+{
+    __shared__ float sh[4];
+    constexpr float kCells = (float)((1 << kKeyBits) - 1);
+    if (threadIdx.x < 32) {                       // reduce the kBoxBlocks partial boxes (cubic cells)
+        float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
+        for (int b = threadIdx.x; b < kBoxBlocks; b += 32) {
+            const float4 l = boxes[2 * b], h = boxes[2 * b + 1];
+            lo[0] = fminf(lo[0], l.x); lo[1] = fminf(lo[1], l.y); lo[2] = fminf(lo[2], l.z);
+            hi[0] = fmaxf(hi[0], h.x); hi[1] = fmaxf(hi[1], h.y); hi[2] = fmaxf(hi[2], h.z);
+        }
+        float ext = 0.f;
+        for (int c = 0; c < 3; ++c) {
+            lo[c] = warp_min(lo[c]); hi[c] = warp_max(hi[c]);
+            ext = fmaxf(ext, hi[c] - lo[c]);
+        }
+        if (threadIdx.x == 0) {
+            sh[0] = lo[0]; sh[1] = lo[1]; sh[2] = lo[2];
+            sh[3] = (ext > 0.f && ext < 3.0e38f) ? kCells / ext : 0.f;
+        }
+    }
+    __syncthreads();
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float4 p = posm[i];
+    const float sc = sh[3];
+    const uint32_t qx = (uint32_t)fminf(fmaxf((p.x - sh[0]) * sc, 0.f), kCells);
+    const uint32_t qy = (uint32_t)fminf(fmaxf((p.y - sh[1]) * sc, 0.f), kCells);
+    const uint32_t qz = (uint32_t)fminf(fmaxf((p.z - sh[2]) * sc, 0.f), kCells);
+    keys[i] = hilbert_key(qx, qy, qz);
+    vals[i] = (uint32_t)i;
+}
+
+// One 1024-thread block per super-group.  gbox[2g] = (lo.xyz, Rmax), gbox[2g+1] = (hi.xyz, 0);
+// sbox likewise per block.
+__global__ void __launch_bounds__(kGroup * kSuper)
+nb_gather_kernel(const float4* __restrict__ posm, const float4* __restrict__ vel, const uint32_t* __restrict__ perm,
+                 int n, const DevState* __restrict__ dev, float4* __restrict__ ps, float4* __restrict__ vs,
+                 float4* __restrict__ gbox, float4* __restrict__ sbox)
+{
+    __shared__ float sh[7][kSuper];
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f}, rmax = 0.f;
+    if (k < n) {
+        const int src = perm ? (int)perm[k] : k;
+        const float4 p = posm[src], v = vel[src];
+        const float R = star_radius(src, dev->n1, dev->R[0], dev->R[1]);
+        ps[k] = make_float4(p.x, p.y, p.z, R);
+        vs[k] = make_float4(v.x, v.y, v.z, p.w);
+        lo[0] = hi[0] = p.x; lo[1] = hi[1] = p.y; lo[2] = hi[2] = p.z; rmax = R;
+    }
+    for (int c = 0; c < 3; ++c) { lo[c] = warp_min(lo[c]); hi[c] = warp_max(hi[c]); }
+    rmax = warp_max(rmax);
+    const int g = blockIdx.x * kSuper + w;
+    if (l == 0) {
+        if ((long long)g * kGroup < n) {
+            gbox[2 * g] = make_float4(lo[0], lo[1], lo[2], rmax);
+            gbox[2 * g + 1] = make_float4(hi[0], hi[1], hi[2], 0.f);
+        }
+        for (int c = 0; c < 3; ++c) { sh[c][w] = lo[c]; sh[3 + c][w] = hi[c]; }
+        sh[6][w] = rmax;
+    }
+    __syncthreads();
+    if (w == 0) {
+        float q[7];
+        for (int c = 0; c < 3; ++c) { q[c] = warp_min(sh[c][l]); q[3 + c] = warp_max(sh[3 + c][l]); }
+        q[6] = warp_max(sh[6][l]);
+        if (l == 0) {
+            sbox[2 * blockIdx.x] = make_float4(q[0], q[1], q[2], q[6]);
+            sbox[2 * blockIdx.x + 1] = make_float4(q[3], q[4], q[5], 0.f);
+        }
+    }
+}
+
+struct ContactArgs {
+    const float4* __restrict__ ps;     // [n] x,y,z,R_star   (Hilbert order)
+    const float4* __restrict__ vs;     // [n] vx,vy,vz,m
+    const uint32_t* __restrict__ perm; // [n] original index of sorted element k (nullptr: identity)
+    const float4* __restrict__ gbox;   // [2*ngroups]
+    const float4* __restrict__ sbox;   // [2*nsuper]
+    float4* __restrict__ out;          // [n] contact acceleration, ORIGINAL index order
+    int n, ngroups, nsuper;
+    float gamma, gamma_beta;           // Eq. 5 / Eq. 6 strengths
+    float v_dead;
+    int lens_mode;
+};
+
+// Squared gap between two axis-aligned boxes (0 if they overlap).
+__device__ __forceinline__ float box_gap2(const float4 alo, const float4 ahi, const float4 blo, const float4 bhi) {
+    const float gx = fmaxf(0.f, fmaxf(alo.x - bhi.x, blo.x - ahi.x));
+    const float gy = fmaxf(0.f, fmaxf(alo.y - bhi.y, blo.y - ahi.y));
+    const float gz = fmaxf(0.f, fmaxf(alo.z - bhi.z, blo.z - ahi.z));
+    return gx * gx + gy * gy + gz * gz;
+}
+
+// The contact term of one (i, j) pair, Eqs. 5/6, added to the fp64
+// accumulators of i:  a_i -= g pi V(r; R_ij) / m_i * d/r  if 0 < r < R_i + R_j  (A2, A3).
+// Evaluated in double throughout (h = 2R - r cancels badly in fp32 near first contact);
+// d is the exact difference of the fp32 coordinates.
+// lens_mode 0: pi V = pi (D - r)^2 (2D + r) / 12 with D = 2 R_ij (factored displaced
+// volume, A1); lens_mode 1: the polynomial as printed (PAPER.md:80), last term r^2/12.
+__device__ __forceinline__ void contact_term(const ContactArgs& a, const float4 pi, const float4 vi,
+                                             const float4 pj, const float4 vj,
+                                             double& ax, double& ay, double& az)
+{
+    const double dx = (double)pj.x - (double)pi.x, dy = (double)pj.y - (double)pi.y, dz = (double)pj.z - (double)pi.z;
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double D = (double)pi.w + (double)pj.w;                   // R_i + R_j = 2 R_ij (A2)
+    if (!(r2 < D * D) || r2 == 0.0) return;                         // not in contact / coincident (A3)
+    const double r = sqrt(r2);
+    const double rinv = 1.0 / r;
+    const double rdot = (dx * ((double)vj.x - (double)vi.x) + dy * ((double)vj.y - (double)vi.y)
+                       + dz * ((double)vj.z - (double)vi.z)) * rinv;
+    const double g = (rdot < -(double)a.v_dead) ? (double)a.gamma : (double)a.gamma_beta;  // Eq. 5 : Eq. 6 (A5)
+    const double kPi = 3.14159265358979323846;
+    double piV;
+    if (a.lens_mode == 0) {
+        const double h = D - r;
+        piV = (kPi / 12.0) * h * h * (2.0 * D + r);
+    } else {
+        const double R = 0.5 * D;
+        piV = kPi * ((4.0 / 3.0) * R * R * R - R * R * r + r * r / 12.0);
+    }
+    const double c = -g * piV / (double)vi.w * rinv;                // vi.w = m_i
+    ax += c * dx; ay += c * dy; az += c * dz;
+}
+
+// Squared gap between a point and an axis-aligned box (0 inside).
+__device__ __forceinline__ float point_gap2(const float4 p, const float4 lo, const float4 hi) {
+    const float gx = fmaxf(0.f, fmaxf(lo.x - p.x, p.x - hi.x));
+    const float gy = fmaxf(0.f, fmaxf(lo.y - p.y, p.y - hi.y));
+    const float gz = fmaxf(0.f, fmaxf(lo.z - p.z, p.z - hi.z));
+    return gx * gx + gy * gy + gz * gz;
+}
+
+constexpr int kCandCap = 128;         // candidate groups buffered per warp before they are processed
+
+// Evaluate the lane's element i against the `cnt` candidate groups listed in cand[]:
+// a group is skipped unless some lane's point is within reach of its box; its 32 elements are
+// staged in the warp's shared-memory slot (coalesced load, broadcast reads).
+__device__ __forceinline__ void contact_candidates(const ContactArgs& a, const int* __restrict__ cand, int cnt,
+                                                   float4* __restrict__ stage, const float4 pi, const float4 vi,
+                                                   bool valid, int lane, double& ax, double& ay, double& az)
+{
+    const float kSlack = 1.0f + 1.0e-5f;
+    for (int q = 0; q < cnt; ++q) {
+        const int jg = cand[q];
+        const float4 lo = a.gbox[2 * jg], hi = a.gbox[2 * jg + 1];
+        const float Db = pi.w + lo.w;
+        if (!__any_sync(0xffffffffu, valid && point_gap2(pi, lo, hi) <= Db * Db * kSlack)) continue;
+        const int j0 = jg * kGroup;
+        const int jn = min(kGroup, a.n - j0);
+        __syncwarp();
+        if (lane < jn) stage[lane] = a.ps[j0 + lane];
+        __syncwarp();
+        for (int t = 0; t < jn; ++t) {
+            const float4 pj = stage[t];
+            const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
+            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+            const float D = pi.w + pj.w;
+            if (r2 <= D * D * kSlack && valid) contact_term(a, pi, vi, pj, a.vs[j0 + t], ax, ay, az);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(kThreads)
+nb_contact_kernel(const __grid_constant__ ContactArgs a)
+{
+    __shared__ int cand_s[kThreads / 32][kCandCap];
+    __shared__ float4 stage_s[kThreads / 32][kGroup];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int ig = (blockIdx.x * kThreads + threadIdx.x) >> 5;     // group of elements i of this warp
+    if (ig >= a.ngroups) return;
+    int* cand = cand_s[wib];
+    float4* stage = stage_s[wib];
+    const int k = ig * kGroup + lane;
+    const bool valid = k < a.n;
+    const float4 pi = valid ? a.ps[k] : make_float4(kFarAway, kFarAway, kFarAway, 0.f);
+    const float4 vi = valid ? a.vs[k] : make_float4(0.f, 0.f, 0.f, 1.f);
+    const float4 ilo = a.gbox[2 * ig], ihi = a.gbox[2 * ig + 1];
+    const float kSlack = 1.0f + 1.0e-5f;                            // the box and fp32 pair tests are pre-filters
+    double ax = 0.0, ay = 0.0, az = 0.0;
+    int cnt = 0;
+
+    for (int sb = 0; sb < a.nsuper; sb += 32) {
+        bool near = false;
+        if (sb + lane < a.nsuper) {
+            const float4 lo = a.sbox[2 * (sb + lane)], hi = a.sbox[2 * (sb + lane) + 1];
+            const float D = ilo.w + lo.w;
+            near = box_gap2(ilo, ihi, lo, hi) <= D * D * kSlack;
+        }
+        unsigned smask = __ballot_sync(0xffffffffu, near);
+        while (smask) {
+            const int s = sb + __ffs(smask) - 1;
+            smask &= smask - 1;
+            const int g = s * kSuper + lane;
+            bool gnear = false;
+            if (g < a.ngroups) {
+                const float4 lo = a.gbox[2 * g], hi = a.gbox[2 * g + 1];
+                const float D = ilo.w + lo.w;
+                gnear = box_gap2(ilo, ihi, lo, hi) <= D * D * kSlack;
+            }
+            const unsigned gmask = __ballot_sync(0xffffffffu, gnear);
+            const int m = __popc(gmask);
+            if (cnt + m > kCandCap) {                               // flush the list before it overflows
+                __syncwarp();
+                contact_candidates(a, cand, cnt, stage, pi, vi, valid, lane, ax, ay, az);
+                cnt = 0;
+                __syncwarp();
+            }
+            if (gnear) cand[cnt + __popc(gmask & ((1u << lane) - 1u))] = g;
+            cnt += m;
+        }
+    }
+    __syncwarp();
+    contact_candidates(a, cand, cnt, stage, pi, vi, valid, lane, ax, ay, az);
+    if (valid) {
+        const int dst = a.perm ? (int)a.perm[k] : k;
+        a.out[dst] = make_float4((float)ax, (float)ay, (float)az, 0.f);
     }
 }
 
