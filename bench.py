@@ -177,7 +177,7 @@ def run_reference(args):
 # ----------------------------------------------------------------------------- own arm
 def ncu_traffic_bytes():
     """dram bytes per force-kernel launch from the committed ncu --set full summary, or None."""
-    path = os.path.join(ROOT, "profiles", "r1_force_kernel_full.md")
+    path = os.path.join(ROOT, "profiles", "r1_gravity_kernel_full.md")
     try:
         for line in open(path):
             if line.startswith("dram_bytes_per_launch"):
