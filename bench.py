@@ -175,9 +175,10 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------- own arm
-def ncu_traffic_bytes():
-    """dram bytes per force-kernel launch from the committed ncu --set full summary, or None."""
-    path = os.path.join(ROOT, "profiles", "r1_gravity_kernel_full.md")
+def ncu_traffic_bytes(kernel):
+    """dram bytes per force-kernel launch from the committed ncu --set full summary of `kernel`, or None."""
+    name = "r1_gravity_sym_kernel_full.md" if "sym" in kernel else "r1_gravity_kernel_full.md"
+    path = os.path.join(ROOT, "profiles", name)
     try:
         for line in open(path):
             if line.startswith("dram_bytes_per_launch"):
@@ -209,7 +210,10 @@ def run_own(args):
     p = params_f32(w.params)
     n = w.n
     stream = torch.cuda.current_stream(dev)
-    sim = nb.Simulation(w.posm, w.vel, w.star, p, device=f"cuda:{local_rank}", stream=stream)
+    path = {"auto": nb.NB_PATH_AUTO, "one-sided": nb.NB_PATH_ONE_SIDED, "symmetric": nb.NB_PATH_SYMMETRIC}[args.path]
+    sim = nb.Simulation(w.posm, w.vel, w.star, p, device=f"cuda:{local_rank}", stream=stream, force_path=path)
+    kernel = nb.nb_force_kernel_name(sim.ctx)
+    symmetric = "sym" in kernel
     flush = torch.empty(L2_FLUSH_BYTES, dtype=torch.uint8, device=dev)
     info = nb.nb_get_launch_info(sim.ctx)
 
@@ -247,9 +251,22 @@ def run_own(args):
     peak_tflops = props.multi_processor_count * FP32_LANES_PER_SM * 2 * sm_max_mhz * 1e6 / 1e12
     achieved = FLOP_PER_INTERACTION * float(n) * n / (k_ms * 1e-3) / 1e12
     step_ms = ms_total / args.steps
+    # What the kernel executes per ordered interaction (FMA-pipe flop + one per MUFU), as opposed to the
+    # 21 flop Eq. 4 itself needs (the convention `achieved` uses).  One-sided kernel: 20.5 + 1.5 (Montgomery
+    # costs 1.5 more multiplies and saves half a MUFU).  Symmetric kernel: one pair evaluation of 26.5 + 1.5
+    # serves two interactions (the super-tiles on the diagonal run one-sided: weight S/N).
+    if symmetric:
+        diag = info["i_per_cta"] / float(n)
+        executed = (1.0 - diag) * 14.0 + diag * 22.0
+    else:
+        executed = 22.0
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-                "frac": achieved / peak_tflops, "traffic": ncu_traffic_bytes(),
-                "kernel": "nb_gravity_kernel<2,256>", "kernel_ms": k_ms,
+                "frac": achieved / peak_tflops, "traffic": ncu_traffic_bytes(kernel),
+                "kernel": kernel, "kernel_ms": k_ms,
+                "executed_flop_per_interaction": executed,
+                "frac_executed": achieved / peak_tflops * executed / FLOP_PER_INTERACTION,
+                "pair_evaluations": "each unordered pair once (Newton's third law)" if symmetric
+                                    else "every ordered pair",
                 "kernel_share_of_step": k_ms / step_ms,
                 "contact_pass_ms": c_ms, "contact_pass_share_of_step": c_ms / step_ms,
                 "interactions_per_s": float(n) * n / (k_ms * 1e-3),
@@ -328,6 +345,8 @@ def main(argv=None):
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--path", choices=["auto", "one-sided", "symmetric"], default="auto",
+                    help="row-a2 kernel (nb_set_force_path); auto = the library's choice")
     ap.add_argument("--impl", choices=["own", "reference"], default="own")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     args = ap.parse_args(argv)

@@ -75,7 +75,8 @@ typedef struct {
 int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream);
 
 /* Bytes of device workspace nb_set_state() needs for a context of n_max elements
- * (cached acceleration, split-j partial sums, device-side step/radius state,
+ * (cached acceleration, partial sums of the gravity kernel -- up to 385 slabs of n float4 for the
+ * symmetric kernel, i.e. ~6.2 KB per element --, device-side step/radius state,
  * reduction scratch, and the contact pass's Hilbert keys, sort scratch, ordered copy and
  * group boxes).  0 if n_max is out of range. */
 size_t nb_workspace_bytes(int64_t n_max);
@@ -119,8 +120,29 @@ int nb_upload_state(nb_ctx* ctx, const float* host_posm, const float* host_vel, 
 int nb_download_state(nb_ctx* ctx, float* host_posm, float* host_vel, float* host_acc);
 
 /* Launch configuration chosen for the bound state (for reports): i-elements per
- * CTA, j-splits P, CTAs of the force kernel, CTAs of the update kernel. */
+ * CTA, j-splits P, CTAs of the force kernel, CTAs of the update kernel (one-sided kernel);
+ * super-tile size S, super-tiles T (= partial-sum slabs), CTAs = T(T+1)/2, CTAs of the update
+ * kernel (symmetric kernel). */
 int nb_get_launch_info(nb_ctx* ctx, int32_t* out4);
+
+/* Which kernel evaluates row a2 (Eq. 4, summed over all pairs).
+ *   NB_PATH_AUTO (default): the symmetric kernel for 32768 <= n <= 2097152, else the one-sided
+ *     kernel (the symmetric kernel is never used above 2097152 elements: its partial sums would
+ *     not fit; NB_PATH_SYMMETRIC then falls back to the one-sided kernel as well).
+ *   NB_PATH_ONE_SIDED: every ORDERED pair (i, j) is evaluated; a CTA owns an (i-block, j-split).
+ *   NB_PATH_SYMMETRIC: every UNORDERED pair is evaluated once and serves both a_i and a_j
+ *     (the force of Eq. 4 is "between elements i and j": F_ij = -F_ji); a CTA owns a pair of
+ *     super-tiles.  Both compute the same sum in a fixed order (bitwise reproducible run to run);
+ *     they differ from each other by fp32 rounding only.
+ * May be called before or after nb_set_state(); NB_ENOMEM if the bound workspace cannot hold the
+ * partial sums of the requested path for the bound n (it always can for n_max >= 32768 or the
+ * default path).  Drops nothing: the cached acceleration stays valid. */
+enum { NB_PATH_AUTO = 0, NB_PATH_ONE_SIDED = 1, NB_PATH_SYMMETRIC = 2 };
+int nb_set_force_path(nb_ctx* ctx, int path);
+
+/* Name (template instantiation) of the row-a2 kernel chosen for the bound state, for reports;
+ * "" if no state is bound.  The string is static. */
+const char* nb_force_kernel_name(nb_ctx* ctx);
 
 /* Kernels launched by this ctx since nb_create() (for bench accounting). */
 int64_t nb_launch_count(nb_ctx* ctx);

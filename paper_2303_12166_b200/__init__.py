@@ -16,10 +16,12 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("NB_LIB_PATH") or os.path.join(HERE, "libnb.so")   # override: development only
 
 NB_OK, NB_EINVAL, NB_ESTATE, NB_ECUDA, NB_ENOMEM, NB_EARCH = 0, -1, -2, -3, -4, -5
+NB_PATH_AUTO, NB_PATH_ONE_SIDED, NB_PATH_SYMMETRIC = 0, 1, 2
 
 EXPORTS = ("nb_create", "nb_workspace_bytes", "nb_set_state", "nb_compute_accel", "nb_step",
            "nb_energy", "nb_get_step", "nb_upload_state", "nb_download_state",
-           "nb_get_launch_info", "nb_launch_count", "nb_time_force_kernel", "nb_time_contact_pass", "nb_destroy", "nb_strerror",
+           "nb_get_launch_info", "nb_set_force_path", "nb_force_kernel_name", "nb_launch_count",
+           "nb_time_force_kernel", "nb_time_contact_pass", "nb_destroy", "nb_strerror",
            "nb_last_cuda_error", "nb_roche_lobe_radius", "nb_l1_distance")
 
 
@@ -73,6 +75,10 @@ def lib() -> C.CDLL:
         L.nb_download_state.argtypes = [vp, vp, vp, vp]
         L.nb_get_launch_info.restype = C.c_int
         L.nb_get_launch_info.argtypes = [vp, C.POINTER(i32)]
+        L.nb_set_force_path.restype = C.c_int
+        L.nb_set_force_path.argtypes = [vp, C.c_int]
+        L.nb_force_kernel_name.restype = C.c_char_p
+        L.nb_force_kernel_name.argtypes = [vp]
         L.nb_launch_count.restype = i64
         L.nb_launch_count.argtypes = [vp]
         L.nb_time_force_kernel.restype = C.c_int
@@ -180,6 +186,14 @@ def nb_get_launch_info(ctx: int) -> Dict[str, int]:
     return dict(i_per_cta=out[0], j_splits=out[1], force_ctas=out[2], update_ctas=out[3])
 
 
+def nb_set_force_path(ctx: int, path: int) -> None:
+    _check(lib().nb_set_force_path(ctx, int(path)), "nb_set_force_path", ctx)
+
+
+def nb_force_kernel_name(ctx: int) -> str:
+    return lib().nb_force_kernel_name(ctx).decode()
+
+
 def nb_launch_count(ctx: int) -> int:
     return int(lib().nb_launch_count(ctx))
 
@@ -213,7 +227,7 @@ class Simulation:
     the kernels of libnb.so do all the work)."""
 
     def __init__(self, posm, vel, star, params: Dict[str, object], device: str = "cuda:0",
-                 stream=None, n_max: Optional[int] = None):
+                 stream=None, n_max: Optional[int] = None, force_path: int = NB_PATH_AUTO):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("paper_2303_12166_b200 needs a CUDA (sm_100) device; there is no CPU fallback")
@@ -232,6 +246,8 @@ class Simulation:
             self.acc = torch.zeros((self.n, 4), dtype=torch.float32, device=self.device)
         self.stream.synchronize()
         self.ctx = nb_create(self.n_max, self.params, self.stream.cuda_stream)
+        if force_path != NB_PATH_AUTO:
+            nb_set_force_path(self.ctx, force_path)
         nb_set_state(self.ctx, self.n, self.posm, self.vel, self.star, self.workspace)
 
     def compute_accel(self):

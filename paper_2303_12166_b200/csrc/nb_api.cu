@@ -28,12 +28,31 @@ struct Plan {           // launch configuration of the gravity kernel for a give
     int nib = 0;        // i blocks
     int njt = 0;        // j tiles
     int nsplit = 1;     // j splits P
+    int sym_S = 0;      // > 0: symmetric kernel with super-tiles of sym_S elements (else the one-sided kernel)
+    int T = 0;          // symmetric kernel: number of super-tiles = slabs of partial sums
 };
 
 constexpr int kCtasPerSM = 8;                      // resident CTAs/SM of nb_gravity_kernel<2, .> (64 registers)
 constexpr int64_t kMaxSplit = 64;
 constexpr int64_t kPartialBudget = (int64_t)128 << 20;   // bytes of split-j partial sums worth keeping in L2
 constexpr int64_t kSortMinN = 8192;                // below this the contact pass takes groups in index order
+
+// Force-path selection (nb_set_force_path).
+enum { kPathAuto = 0, kPathOneSided = 1, kPathSymmetric = 2 };
+constexpr int64_t kSymMinN = 32768;               // auto: symmetric kernel from here on (enough CTAs to fill the SMs)
+constexpr int64_t kSymMaxN = (int64_t)1 << 21;    // ... up to here: its T slabs of n float4 reach 17 GB at 2M elements
+
+// Super-tile size of the symmetric kernel for n elements: its T = ceil(n/S) slabs of n float4
+// partial sums cost memory and one extra pass, so S grows with n.
+int sym_tile(int64_t n)
+{
+    if (n < 196608) return 512;       // T <= 384 in every band
+    if (n < 393216) return 1024;
+    if (n < 786432) return 2048;
+    return 4096;
+}
+
+int64_t sym_slabs(int64_t n) { const int64_t S = sym_tile(n); return (n + S - 1) / S; }
 
 // Largest number of j splits allowed for n elements (bounds the partial-sum slabs).
 int64_t max_split(int64_t n)
@@ -51,15 +70,29 @@ int64_t partial_elems_bound(int64_t n_max)
     const int64_t a = (kMaxSplit + 1) * n_max;
     const int64_t b1 = 9 * n_max, b2 = kPartialBudget / 16 + n_max;
     const int64_t b = b1 > b2 ? b1 : b2;
-    return a < b ? a : b;
+    int64_t r = a < b ? a : b;
+    // symmetric kernel: (T(n) + 1) n, largest just below each change of the super-tile size
+    const int64_t top = n_max < kSymMaxN ? n_max : kSymMaxN;
+    const int64_t tops[3] = {196607, 393215, 786431};
+    int64_t probes[4] = {top, top, top, top};
+    for (int k = 0; k < 3; ++k) if (tops[k] < top) probes[k + 1] = tops[k];
+    for (int64_t n : probes) {
+        const int64_t e = (sym_slabs(n) + 1) * n;
+        if (e > r) r = e;
+    }
+    return r;
 }
 
 // P j-splits give nib*P equal CTAs that run in rounds of `slots` resident CTAs: the cost is
 // rounds x (tiles per split + a per-CTA prologue), with a small term for the ragged end of
 // the last round (CTAs drift apart, so more rounds end more evenly).
-Plan make_plan(int64_t n, int num_sms)
+Plan make_plan(int64_t n, int num_sms, int path)
 {
     Plan p;
+    if ((path == kPathSymmetric || (path == kPathAuto && n >= kSymMinN)) && n <= kSymMaxN) {
+        p.sym_S = sym_tile(n);
+        p.T = (int)sym_slabs(n);
+    }
     p.I = 2;
     p.TJ = n >= 16384 ? 256 : 128;
     const int ib = kThreads * p.I;
@@ -125,6 +158,7 @@ struct nb_ctx {
     Layout lay{};
     Plan plan{};
     bool have_state = false, have_acc = false;
+    int path = kPathAuto;
     int last_cuda = 0;
     int64_t launches = 0;
 
@@ -140,7 +174,8 @@ struct nb_ctx {
     float4* sbox() const { return reinterpret_cast<float4*>(ws + lay.off_sbox); }
     float4* boxes() const { return reinterpret_cast<float4*>(ws + lay.off_boxes); }
     bool contact_on() const { return prm.gamma > 0.f; }
-    int nslabs() const { return plan.nsplit + (contact_on() ? 1 : 0); }   // slabs nb_reduce_update_kernel sums
+    int ngrav() const { return plan.sym_S ? plan.T : plan.nsplit; }       // gravity slabs
+    int nslabs() const { return ngrav() + (contact_on() ? 1 : 0); }       // slabs nb_reduce_update_kernel sums
 };
 
 #define NB_CUDA(ctx, call)                                   \
@@ -169,9 +204,32 @@ bool params_ok(const nb_params* p)
     return true;
 }
 
-// Row a2: partial gravitational accelerations of all (i-block, j-split) pairs -> part[0..P-1][n]
+// The three instantiations of the symmetric kernel: <S, H, threads, CTAs/SM, packed reaction, Montgomery>.
+#define NB_SYM_512  nb_gravity_sym_kernel<512, 2, 128, 4, true, true>
+#define NB_SYM_1024 nb_gravity_sym_kernel<1024, 2, 256, 2, true, true>
+#define NB_SYM_2048 nb_gravity_sym_kernel<2048, 2, 256, 2, true, true>
+#define NB_SYM_4096 nb_gravity_sym_kernel<4096, 2, 256, 2, true, true>
+
+// Row a2: partial gravitational accelerations -> part[0..ngrav-1][n]
+//   symmetric kernel: one CTA per pair of super-tiles, part[Y][e] = a_e due to super-tile Y
+//   one-sided kernel: one CTA per (i-block, j-split), part[p][i] = a_i due to split p
 int launch_gravity(nb_ctx* c)
 {
+    if (c->plan.sym_S) {
+        SymArgs sa;
+        sa.posm = c->posm; sa.part = c->part(); sa.n = (int)c->n; sa.T = c->plan.T;
+        sa.G = c->prm.G; sa.eps = c->prm.eps;
+        const long long T = c->plan.T;
+        const int grid = (int)(T * (T + 1) / 2);
+        const int smem = kSymSmemPerElem * c->plan.sym_S;
+        if (c->plan.sym_S == 512)       NB_SYM_512<<<grid, 128, smem, c->stream>>>(sa);
+        else if (c->plan.sym_S == 1024) NB_SYM_1024<<<grid, 256, smem, c->stream>>>(sa);
+        else if (c->plan.sym_S == 2048) NB_SYM_2048<<<grid, 256, smem, c->stream>>>(sa);
+        else                            NB_SYM_4096<<<grid, 256, smem, c->stream>>>(sa);
+        c->launches++;
+        NB_CUDA(c, cudaGetLastError());
+        return NB_OK;
+    }
     GravArgs ga;
     ga.posm = c->posm; ga.part = c->part();
     ga.n = (int)c->n; ga.nib = c->plan.nib; ga.nsplit = c->plan.nsplit; ga.njt = c->plan.njt;
@@ -209,7 +267,7 @@ int launch_contact(nb_ctx* c)
     c->launches++;
     ContactArgs ca;
     ca.ps = c->ps(); ca.vs = c->vs(); ca.perm = perm; ca.gbox = c->gbox(); ca.sbox = c->sbox();
-    ca.out = c->part() + (size_t)c->plan.nsplit * c->n;
+    ca.out = c->part() + (size_t)c->ngrav() * c->n;
     ca.n = n; ca.ngroups = ngroups; ca.nsuper = nsuper;
     ca.gamma = c->prm.gamma; ca.gamma_beta = c->prm.gamma * c->prm.beta;
     ca.v_dead = c->prm.v_dead; ca.lens_mode = c->prm.lens_mode;
@@ -297,6 +355,14 @@ int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream
     c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     c->num_sms = sms > 0 ? sms : kNumSMsFallback;
     c->lay = make_layout(n_max);
+    // the symmetric kernel's shared memory is dynamic (112 KB at S = 4096)
+    if (cudaFuncSetAttribute(NB_SYM_512, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 512) != cudaSuccess ||
+        cudaFuncSetAttribute(NB_SYM_1024, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(NB_SYM_2048, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 2048) != cudaSuccess ||
+        cudaFuncSetAttribute(NB_SYM_4096, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 4096) != cudaSuccess) {
+        delete c;
+        return NB_ECUDA;
+    }
     {   // the radix sort's scratch must fit the slice the layout reserves for it
         size_t need = 0;
         cub::DoubleBuffer<unsigned long long> dk(nullptr, nullptr);
@@ -346,8 +412,8 @@ int nb_set_state(nb_ctx* c, int64_t n, float* posm, float* vel, const int32_t* s
     c->n1 = h.n1;
     c->posm = reinterpret_cast<float4*>(posm);
     c->vel = reinterpret_cast<float4*>(vel);
-    c->plan = make_plan(n, c->num_sms);
-    if ((int64_t)(c->plan.nsplit + 1) * n > partial_elems_bound(c->n_max)) return NB_ENOMEM;
+    c->plan = make_plan(n, c->num_sms, c->path);
+    if ((int64_t)(c->ngrav() + 1) * n > partial_elems_bound(c->n_max)) return NB_ENOMEM;
     c->have_state = true;
     return NB_OK;
 }
@@ -481,11 +547,40 @@ int nb_get_launch_info(nb_ctx* c, int32_t* out4)
 {
     if (!c || !out4) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
-    out4[0] = kThreads * c->plan.I;
-    out4[1] = c->plan.nsplit;
-    out4[2] = c->plan.nib * c->plan.nsplit;
+    if (c->plan.sym_S) {
+        out4[0] = c->plan.sym_S;
+        out4[1] = c->plan.T;
+        out4[2] = (int)((long long)c->plan.T * (c->plan.T + 1) / 2);
+    } else {
+        out4[0] = kThreads * c->plan.I;
+        out4[1] = c->plan.nsplit;
+        out4[2] = c->plan.nib * c->plan.nsplit;
+    }
     out4[3] = (int)((c->n + 255) / 256);
     return NB_OK;
+}
+
+int nb_set_force_path(nb_ctx* c, int path)
+{
+    if (!c || path < kPathAuto || path > kPathSymmetric) return NB_EINVAL;
+    if (c->have_state) {
+        const Plan p = make_plan(c->n, c->num_sms, path);
+        const int64_t ngrav = p.sym_S ? p.T : p.nsplit;
+        if ((ngrav + 1) * c->n > partial_elems_bound(c->n_max)) return NB_ENOMEM;
+        c->plan = p;
+    }
+    c->path = path;
+    return NB_OK;
+}
+
+const char* nb_force_kernel_name(nb_ctx* c)
+{
+    if (!c || !c->have_state) return "";
+    if (c->plan.sym_S == 512) return "nb_gravity_sym_kernel<512,2,128,4,1,1>";
+    if (c->plan.sym_S == 1024) return "nb_gravity_sym_kernel<1024,2,256,2,1,1>";
+    if (c->plan.sym_S == 2048) return "nb_gravity_sym_kernel<2048,2,256,2,1,1>";
+    if (c->plan.sym_S) return "nb_gravity_sym_kernel<4096,2,256,2,1,1>";
+    return c->plan.TJ == 256 ? "nb_gravity_kernel<2,256>" : "nb_gravity_kernel<2,128>";
 }
 
 int64_t nb_launch_count(nb_ctx* c) { return c ? c->launches : 0; }

@@ -63,6 +63,11 @@ __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
     f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
 }
 
+// add2 that the compiler may neither move nor fold (see sym_sweep).
+__device__ __forceinline__ f32x2 add2v(f32x2 a, f32x2 b) {
+    f32x2 d; asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
+
 // Radius of the star an element index belongs to (star 0 first, then star 1).
 __device__ __forceinline__ float star_radius(int idx, int n1, float R0, float R1) {
     return idx < n1 ? R0 : R1;
@@ -239,6 +244,252 @@ nb_gravity_kernel(const __grid_constant__ GravArgs a)
     for (int k = 0; k < I; ++k) {
         const int i = ibase + k * kThreads;
         if (i < a.n) out[i] = make_float4((float)accx[k], (float)accy[k], (float)accz[k], 0.f);
+    }
+}
+
+// ---------------------------------------------------------------------------
+// Row a2 for large N: the same sum with every UNORDERED pair evaluated once.
+//
+// Eq. 4 is a force "between elements i and j": F_ij = -F_ji, so the geometric
+// factor c = 1/(r (r+eps)^2) and the difference d of a pair serve both a_i += G m_j c d and
+// a_j -= G m_i c d.  Elements are cut into super-tiles of S; one CTA owns one pair of
+// super-tiles (A <= B).  Its 8 warps each keep 64 elements i of A in registers (two per lane, one
+// packed pair) and walk the tiles of 64 elements j of B.  Inside a tile the warp ROTATES: at step
+// k lane l meets slots (l+k)&31 and 32+((l+k)&31) (conflict-free LDS.128), accumulates a_i in its
+// own registers and the pair's reaction in six scalar registers that travel with the slots
+// (SHFL to lane l-1 after every step); after 32 steps the lane holds the finished sums of slots l
+// and 32+l over the warp's 64 elements i and adds them to the CTA's shared-memory array.  The
+// warps of a CTA are skewed over different tiles and meet at a barrier after every tile, so the
+// shared-memory sums have a fixed order: results are bitwise reproducible.
+// Per lane and step (2 i x 2 j = 4 pairs = 8 interactions): the 27 packed instructions of the
+// one-sided loop (FADD2 x6, FFMA2 x6+2, FMUL2 x9, FFMA2 x6 -- see above) give c and a_i, 12 scalar FFMA
+// add the reaction, 6 SHFL rotate it: 39 FMA-pipe instructions per 8 interactions instead of
+// 54, and 0.75 MUFU per interaction instead of 1.5.
+// Output: part[Y][e] = acceleration of element e due to the elements of super-tile Y (every
+// (Y, tile of e) combination is written by exactly one CTA; the diagonal CTAs (A == B) run the
+// one-sided loop).  Super-tiles of one mass take the mass out of the loop, as in
+// the one-sided kernel; other pairs of super-tiles multiply c by G m_j and G m_i per pair.
+struct SymArgs {
+    const float4* __restrict__ posm;   // [n] x,y,z,m
+    float4* __restrict__ part;         // [T][n]
+    int n, T;                          // T = ceil(n / S) super-tiles
+    float G, eps;
+};
+
+constexpr int kSymSmemPerElem = 28;    // dynamic shared memory of the symmetric kernel: (16 + 3*4) bytes x S
+
+template <int H, bool UNI, bool SYM, bool JP, bool MONT>
+__device__ __forceinline__ void sym_step(const float4 p0, const float4 p1,
+                                         const f32x2 (&nxi)[H], const f32x2 (&nyi)[H], const f32x2 (&nzi)[H],
+                                         const f32x2 (&gmi)[H], const f32x2 eps2,
+                                         f32x2 (&ax)[H], f32x2 (&ay)[H], f32x2 (&az)[H],
+                                         float (&ja)[3], float (&jb)[3])
+{
+    const f32x2 tiny2 = pk2(kTinyR2, kTinyR2);
+    f32x2 ga[3], gb[3];                                                    // JP: packed reaction of this step
+#pragma unroll
+    for (int h = 0; h < H; ++h) {
+        const f32x2 dx0 = add2(pk2(p0.x, p0.x), nxi[h]), dy0 = add2(pk2(p0.y, p0.y), nyi[h]), dz0 = add2(pk2(p0.z, p0.z), nzi[h]);
+        const f32x2 dx1 = add2(pk2(p1.x, p1.x), nxi[h]), dy1 = add2(pk2(p1.y, p1.y), nyi[h]), dz1 = add2(pk2(p1.z, p1.z), nzi[h]);
+        f32x2 r20 = fma2(dx0, dx0, tiny2); r20 = fma2(dy0, dy0, r20); r20 = fma2(dz0, dz0, r20);
+        f32x2 r21 = fma2(dx1, dx1, tiny2); r21 = fma2(dy1, dy1, r21); r21 = fma2(dz1, dz1, r21);
+        float a0, b0, a1, b1;
+        unpk2(r20, a0, b0); unpk2(r21, a1, b1);
+        const f32x2 ri0 = pk2(rsqrt_approx(a0), rsqrt_approx(b0));         // 1/r
+        const f32x2 ri1 = pk2(rsqrt_approx(a1), rsqrt_approx(b1));
+        const f32x2 s0 = fma2(r20, ri0, eps2), s1 = fma2(r21, ri1, eps2);   // r + eps
+        const f32x2 t0 = mul2(s0, s0), t1 = mul2(s1, s1);                   // (r + eps)^2
+        f32x2 c0, c1;                                                      // 1/(r (r+eps)^2)   Eq. 4
+        if (MONT) {
+            const f32x2 P = mul2(t0, t1);
+            float pl, ph;
+            unpk2(P, pl, ph);
+            const f32x2 iP = pk2(rcp_approx(pl), rcp_approx(ph));          // one RCP per two pairs
+            const f32x2 k0 = mul2(t1, ri0), k1 = mul2(t0, ri1);
+            c0 = mul2(iP, k0); c1 = mul2(iP, k1);
+        } else {
+            float l0, h0, l1, h1;
+            unpk2(t0, l0, h0); unpk2(t1, l1, h1);
+            c0 = mul2(ri0, pk2(rcp_approx(l0), rcp_approx(h0)));
+            c1 = mul2(ri1, pk2(rcp_approx(l1), rcp_approx(h1)));
+        }
+        f32x2 ci0 = c0, ci1 = c1, cj0 = c0, cj1 = c1;
+        if (!UNI) {
+            ci0 = mul2(c0, pk2(p0.w, p0.w)); ci1 = mul2(c1, pk2(p1.w, p1.w));   // G m_j for a_i
+            if (SYM) { cj0 = mul2(c0, gmi[h]); cj1 = mul2(c1, gmi[h]); }        // G m_i for a_j
+        }
+        ax[h] = fma2(ci0, dx0, ax[h]); ay[h] = fma2(ci0, dy0, ay[h]); az[h] = fma2(ci0, dz0, az[h]);
+        ax[h] = fma2(ci1, dx1, ax[h]); ay[h] = fma2(ci1, dy1, ay[h]); az[h] = fma2(ci1, dz1, az[h]);
+        if (SYM && !JP) {                                                  // reaction: a_j -= [G m_i] c d
+            float cl, ch, dl, dh;
+            unpk2(cj0, cl, ch);
+            unpk2(dx0, dl, dh); ja[0] = fmaf(cl, dl, ja[0]); ja[0] = fmaf(ch, dh, ja[0]);
+            unpk2(dy0, dl, dh); ja[1] = fmaf(cl, dl, ja[1]); ja[1] = fmaf(ch, dh, ja[1]);
+            unpk2(dz0, dl, dh); ja[2] = fmaf(cl, dl, ja[2]); ja[2] = fmaf(ch, dh, ja[2]);
+            unpk2(cj1, cl, ch);
+            unpk2(dx1, dl, dh); jb[0] = fmaf(cl, dl, jb[0]); jb[0] = fmaf(ch, dh, jb[0]);
+            unpk2(dy1, dl, dh); jb[1] = fmaf(cl, dl, jb[1]); jb[1] = fmaf(ch, dh, jb[1]);
+            unpk2(dz1, dl, dh); jb[2] = fmaf(cl, dl, jb[2]); jb[2] = fmaf(ch, dh, jb[2]);
+        }
+        if (SYM && JP) {
+            if (h == 0) {
+                ga[0] = mul2(cj0, dx0); ga[1] = mul2(cj0, dy0); ga[2] = mul2(cj0, dz0);
+                gb[0] = mul2(cj1, dx1); gb[1] = mul2(cj1, dy1); gb[2] = mul2(cj1, dz1);
+            } else {
+                ga[0] = fma2(cj0, dx0, ga[0]); ga[1] = fma2(cj0, dy0, ga[1]); ga[2] = fma2(cj0, dz0, ga[2]);
+                gb[0] = fma2(cj1, dx1, gb[0]); gb[1] = fma2(cj1, dy1, gb[1]); gb[2] = fma2(cj1, dz1, gb[2]);
+            }
+        }
+    }
+    if (SYM && JP) {
+#pragma unroll
+        for (int c = 0; c < 3; ++c) {
+            float l, h2;
+            unpk2(ga[c], l, h2); ja[c] = (ja[c] + l) + h2;
+            unpk2(gb[c], l, h2); jb[c] = (jb[c] + l) + h2;
+        }
+    }
+}
+
+// All tiles of super-tile B (in shared memory) against the warp's 64 H elements i, for every
+// round of elements i of super-tile A.
+template <int S, int H, int NT, bool JP, bool MONT, bool UNI, bool SYM>
+__device__ __forceinline__ void sym_sweep(const SymArgs& a, const int A, const int B, const float4* __restrict__ jpos,
+                                          float* __restrict__ jax, float* __restrict__ jay, float* __restrict__ jaz,
+                                          const double scale_i)
+{
+    constexpr int NW = NT / 32;
+    constexpr int NJT = S / 64;                      // tiles of 64 elements j
+    constexpr int SKEW = NJT / NW;                   // the warps of a CTA work on different tiles
+    constexpr int IPR = NW * 64 * H;                 // elements i per round
+    static_assert(S % (64 * NW) == 0 && S % IPR == 0, "every warp needs its own tile at every step");
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int src = (lane + 1) & 31;
+    const f32x2 eps2 = pk2(a.eps, a.eps);
+    float4* __restrict__ out = a.part + (size_t)B * a.n;
+
+#pragma unroll 1
+    for (int r = 0; r < S / IPR; ++r) {
+        const int ibase = A * S + r * IPR + warp * (64 * H) + lane;
+        f32x2 nxi[H], nyi[H], nzi[H], gmi[H], rx[H], ry[H], rz[H];
+#pragma unroll
+        for (int h = 0; h < H; ++h) {
+            const int i0 = ibase + h * 64, i1 = i0 + 32;
+            float4 q0 = make_float4(kFarAway, kFarAway, kFarAway, 0.f), q1 = q0;
+            if (i0 < a.n) q0 = a.posm[i0];
+            if (i1 < a.n) q1 = a.posm[i1];
+            nxi[h] = pk2(-q0.x, -q1.x); nyi[h] = pk2(-q0.y, -q1.y); nzi[h] = pk2(-q0.z, -q1.z);
+            gmi[h] = pk2(a.G * q0.w, a.G * q1.w);
+            // define each packed pair by a packed instruction, so that it lives in one aligned
+            // register pair for the whole sweep (otherwise ptxas keeps the halves where the loads
+            // put them and re-packs them with two MOVs at every use)
+            const f32x2 zero2 = pk2(0.f, 0.f);
+            nxi[h] = add2v(nxi[h], zero2); nyi[h] = add2v(nyi[h], zero2); nzi[h] = add2v(nzi[h], zero2);
+            gmi[h] = add2v(gmi[h], zero2);
+            rx[h] = ry[h] = rz[h] = pk2(0.f, 0.f);
+        }
+
+#pragma unroll 1
+        for (int q = 0; q < NJT; ++q) {
+            const int tile = (q + warp * SKEW) & (NJT - 1);
+            const float4* __restrict__ tp = jpos + tile * 64;
+            f32x2 ax[H], ay[H], az[H];
+#pragma unroll
+            for (int h = 0; h < H; ++h) ax[h] = ay[h] = az[h] = pk2(0.f, 0.f);
+            float ja[3] = {0.f, 0.f, 0.f}, jb[3] = {0.f, 0.f, 0.f};
+#pragma unroll 2
+            for (int k = 0; k < 32; ++k) {
+                const int slot = (lane + k) & 31;
+                sym_step<H, UNI, SYM, JP, MONT>(tp[slot], tp[32 + slot], nxi, nyi, nzi, gmi, eps2, ax, ay, az, ja, jb);
+                if (SYM) {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        ja[c] = __shfl_sync(0xffffffffu, ja[c], src);
+                        jb[c] = __shfl_sync(0xffffffffu, jb[c], src);
+                    }
+                }
+            }
+#pragma unroll
+            for (int h = 0; h < H; ++h) {            // short fp32 chains: 64 terms per tile, then S/64 tile sums
+                rx[h] = add2(rx[h], ax[h]); ry[h] = add2(ry[h], ay[h]); rz[h] = add2(rz[h], az[h]);
+            }
+            if (SYM) {                               // after 32 rotations lane l holds slots l and 32+l
+                const int e = tile * 64 + lane;
+                jax[e] += ja[0]; jay[e] += ja[1]; jaz[e] += ja[2];
+                jax[e + 32] += jb[0]; jay[e + 32] += jb[1]; jaz[e + 32] += jb[2];
+                __syncthreads();                     // fixed order of the shared-memory sums
+            }
+        }
+#pragma unroll
+        for (int h = 0; h < H; ++h) {
+            const int i0 = ibase + h * 64, i1 = i0 + 32;
+            float xl, xh, yl, yh, zl, zh;
+            unpk2(rx[h], xl, xh); unpk2(ry[h], yl, yh); unpk2(rz[h], zl, zh);
+            if (i0 < a.n) out[i0] = make_float4((float)(scale_i * (double)xl), (float)(scale_i * (double)yl),
+                                                (float)(scale_i * (double)zl), 0.f);
+            if (i1 < a.n) out[i1] = make_float4((float)(scale_i * (double)xh), (float)(scale_i * (double)yh),
+                                                (float)(scale_i * (double)zh), 0.f);
+        }
+    }
+}
+
+template <int S, int H, int NT, int MINB, bool JP, bool MONT>
+__global__ void __launch_bounds__(NT, MINB)
+nb_gravity_sym_kernel(const __grid_constant__ SymArgs a)
+{
+    extern __shared__ float4 sym_smem[];             // S float4 + 3 S float = 28 S bytes (dynamic: 56 KB at S = 2048)
+    float4* __restrict__ jpos = sym_smem;
+    float* __restrict__ jax = reinterpret_cast<float*>(sym_smem + S);
+    float* __restrict__ jay = jax + S;
+    float* __restrict__ jaz = jay + S;
+    const int tid = threadIdx.x;
+
+    // block -> (A, B): the T(T-1)/2 off-diagonal pairs row by row, then the T diagonal ones
+    int A, B;
+    {
+        const long long T = a.T, M = T * (T - 1) / 2, b = blockIdx.x;
+        if (b >= M) { A = B = (int)(b - M); }
+        else {
+            const double t2 = 2.0 * (double)T - 1.0;
+            long long r = (long long)((t2 - sqrt(t2 * t2 - 8.0 * (double)b)) * 0.5);
+            if (r < 0) r = 0;
+            while (r > 0 && r * (2 * T - r - 1) / 2 > b) --r;
+            while ((r + 1) * (2 * T - r - 2) / 2 <= b) ++r;
+            A = (int)r;
+            B = (int)(b - r * (2 * T - r - 1) / 2 + r + 1);
+        }
+    }
+
+    // stage super-tile B (G folded into m_j), clear its sums, and find out whether A and B
+    // are each made of one mass
+    const float mB = a.posm[min(B * S, a.n - 1)].w, mA = a.posm[min(A * S, a.n - 1)].w;
+    bool u = true;
+    for (int e = tid; e < S; e += NT) {
+        const int j = B * S + e, i = A * S + e;
+        float4 p = make_float4(kFarAway, kFarAway, kFarAway, 0.f);
+        if (j < a.n) { p = a.posm[j]; u = u && (p.w == mB); p.w *= a.G; } else u = false;
+        if (i < a.n) u = u && (a.posm[i].w == mA); else u = false;
+        jpos[e] = p;
+        jax[e] = 0.f; jay[e] = 0.f; jaz[e] = 0.f;
+    }
+    const int uni = __syncthreads_and(u ? 1 : 0);
+
+    if (A == B) {
+        if (uni) sym_sweep<S, H, NT, JP, MONT, true, false>(a, A, B, jpos, jax, jay, jaz, (double)(a.G * mB));
+        else     sym_sweep<S, H, NT, JP, MONT, false, false>(a, A, B, jpos, jax, jay, jaz, 1.0);
+        return;
+    }
+    if (uni) sym_sweep<S, H, NT, JP, MONT, true, true>(a, A, B, jpos, jax, jay, jaz, (double)(a.G * mB));
+    else     sym_sweep<S, H, NT, JP, MONT, false, true>(a, A, B, jpos, jax, jay, jaz, 1.0);
+
+    // reaction sums of super-tile B due to super-tile A (sign: a_j -= ...)
+    const double scale_j = uni ? -(double)(a.G * mA) : -1.0;
+    float4* __restrict__ outj = a.part + (size_t)A * a.n;
+    for (int e = tid; e < S; e += NT) {
+        const int j = B * S + e;
+        if (j < a.n)
+            outj[j] = make_float4((float)(scale_j * (double)jax[e]), (float)(scale_j * (double)jay[e]),
+                                  (float)(scale_j * (double)jaz[e]), 0.f);
     }
 }
 

@@ -24,8 +24,8 @@ def _sim(nb, w, p=None, **kw):
     return nb.Simulation(w.posm, w.vel, w.star, p or params_f32(w.params), **kw)
 
 
-def _gpu_accel(nb, w, p):
-    s = _sim(nb, w, p)
+def _gpu_accel(nb, w, p, **kw):
+    s = _sim(nb, w, p, **kw)
     a = s.compute_accel()
     s.synchronize()
     out = a.cpu().numpy().astype(np.float64)
@@ -35,9 +35,9 @@ def _gpu_accel(nb, w, p):
     return out[:, :3], info
 
 
-def _check_accel(nb, w, p=None, rows=None, tol=ACC_TOL, contacts_per_element=5):
+def _check_accel(nb, w, p=None, rows=None, tol=ACC_TOL, contacts_per_element=5, **kw):
     p = p or params_f32(w.params)
-    a_gpu, info = _gpu_accel(nb, w, p)
+    a_gpu, info = _gpu_accel(nb, w, p, **kw)
     assert np.isfinite(a_gpu).all()
     a_or, kap, dl = oracle.accel(w.posm, w.vel, w.posm[:, 3], w.star, p["R_start"], p, rows=rows, want_diag=True)
     sel = np.arange(w.n) if rows is None else rows
@@ -91,6 +91,88 @@ def test_accel_ragged_and_degenerate_sizes(nb, n1, n2):
     w.posm, w.vel, w.star = w.posm[keep].copy(), w.vel[keep].copy(), w.star[keep].copy()
     assert w.n == n1 + n2
     _check_accel(nb, w)
+
+
+# ---- the symmetric gravity kernel (every unordered pair once; default for n >= 32768) ----------
+def _ragged(n1, n2, seed=5, **over):
+    kw = dict(name="r", seed=seed, n1=n1, n2=n2, shape="uniform", radius1=1.0, radius2=0.6,
+              q=0.5, a=3.0, eps=0.01, dt=1e-3, nsteps=0)
+    kw.update(over)
+    return make_binary(**kw)
+
+
+@pytest.mark.parametrize("n1,n2", [(1, 1), (31, 2), (1000, 777), (512, 512), (513, 700), (5000, 4321), (16384, 1),
+                                    (17000, 3001), (40000, 25537)])
+def test_symmetric_path_full_parity_ragged_sizes(nb, n1, n2):
+    """The symmetric kernel forced at sizes below its default threshold and off its 512-element
+    super-tiles (padding elements, a star boundary inside a super-tile -> general-mass loop), against
+    the full oracle."""
+    w = _ragged(n1, n2)
+    _check_accel(nb, w, force_path=nb.NB_PATH_SYMMETRIC)
+
+
+@pytest.mark.parametrize("idx", [1, 2])
+def test_symmetric_path_small_configs(nb, idx):
+    """Config 2 has lognormal masses: every super-tile takes the per-pair mass multiplies."""
+    _check_accel(nb, make_config(idx), force_path=nb.NB_PATH_SYMMETRIC)
+
+
+@pytest.mark.parametrize("override", [dict(gamma=0.0), dict(eps=0.0), dict(G=0.0), dict(G=2.5, eps=0.05)])
+def test_symmetric_path_parameter_variants(nb, override):
+    w = make_config(1)
+    p = params_f32(dict(w.params, **override))
+    _check_accel(nb, w, p, force_path=nb.NB_PATH_SYMMETRIC)
+
+
+def test_symmetric_path_zero_mass_and_mixed_tiles(nb):
+    w = _ragged(3000, 2000, seed=9)
+    rng = np.random.default_rng(4)
+    w.posm[::7, 3] = 0.0                                         # massless tracers inside uniform tiles
+    w.posm[1024:2048, 3] *= rng.lognormal(0.0, 0.3, 1024).astype(np.float32)
+    p = params_f32(dict(w.params, gamma=0.0))                    # (the contact term divides by m_i)
+    _check_accel(nb, w, p, force_path=nb.NB_PATH_SYMMETRIC)
+
+
+def test_default_path_and_both_paths_agree_at_full_size(nb):
+    """Config 3 (N = 65,536): the default is the symmetric kernel; the one-sided kernel gives the
+    same accelerations up to fp32 rounding, and a sample of its rows matches the oracle too."""
+    w = make_config(3)
+    p = params_f32(w.params)
+    s = _sim(nb, w, p)
+    assert nb.nb_force_kernel_name(s.ctx).startswith("nb_gravity_sym_kernel<512")
+    a_sym = s.compute_accel().cpu().numpy().astype(np.float64)[:, :3]
+    nb.nb_set_force_path(s.ctx, nb.NB_PATH_ONE_SIDED)
+    assert nb.nb_force_kernel_name(s.ctx) == "nb_gravity_kernel<2,256>"
+    a_one = s.compute_accel().cpu().numpy().astype(np.float64)[:, :3]
+    nb.nb_set_force_path(s.ctx, nb.NB_PATH_AUTO)
+    a_sym2 = s.compute_accel().cpu().numpy().astype(np.float64)[:, :3]
+    s.close()
+    assert np.array_equal(a_sym, a_sym2)                          # fixed summation order
+    d = np.linalg.norm(a_sym - a_one, axis=1) / np.linalg.norm(a_one, axis=1)
+    assert d.max() < 1e-5
+    _check_accel(nb, w, p, rows=_sample(w.n, 1024, 5), force_path=nb.NB_PATH_ONE_SIDED)
+
+
+@pytest.mark.parametrize("n,name", [(32768, "<512"), (200000, "<1024"), (400000, "<2048")])
+def test_symmetric_tile_bands(nb, n, name):
+    """One size in each super-tile band below config 5's (S = 512, 1024, 2048; 4096 is config 5),
+    ragged against the band's tile, sampled rows against the oracle."""
+    w = _ragged(n - n // 3, n // 3, seed=21, eps=0.004)
+    p = params_f32(w.params)
+    s = _sim(nb, w, p)
+    assert name in nb.nb_force_kernel_name(s.ctx)
+    s.close()
+    _check_accel(nb, w, p, rows=_sample(w.n, 512, n))
+
+
+def test_force_path_argument_errors(nb):
+    w = make_config(1)
+    s = _sim(nb, w)
+    assert nb.lib().nb_set_force_path(s.ctx, 3) == nb.NB_EINVAL
+    assert nb.lib().nb_set_force_path(s.ctx, -1) == nb.NB_EINVAL
+    assert nb.lib().nb_set_force_path(None, 0) == nb.NB_EINVAL
+    assert nb.lib().nb_force_kernel_name(None) == b""
+    s.close()
 
 
 def test_single_element_has_zero_acceleration(nb):
@@ -353,11 +435,13 @@ def test_long_run_invariants_config1(nb):
     assert e1["step"] == 300
 
 
-def test_results_are_bitwise_reproducible(nb):
+@pytest.mark.parametrize("path", [1, 2])
+def test_results_are_bitwise_reproducible(nb, path):
+    """Both gravity kernels sum in a fixed order (no atomics): two runs give the same bits."""
     w = make_config(2, scale=0.5)
     outs = []
     for _ in range(2):
-        s = _sim(nb, w)
+        s = _sim(nb, w, force_path=path)
         s.step(3)
         a = s.compute_accel()
         s.synchronize()
