@@ -1,7 +1,8 @@
 // nb_kernels.cuh -- sm_100a kernels of the all-pairs binary-star element model.
 //
 // Hot path:
-//   a2     nb_gravity_kernel        all-pairs Eq. 4 gravity, every ordered pair
+//   a2     nb_gravity_sym_kernel    all-pairs Eq. 4 gravity, every unordered pair once
+//          nb_gravity_kernel        the same sum over every ordered pair (small and very large n)
 //   a3     nb_contact_kernel        contact terms of Eqs. 5/6 for exactly the
 //                                   pairs with r < R_i + R_j, found through Hilbert-ordered groups
 //                                   of 32 elements and their bounding boxes
