@@ -16,9 +16,12 @@
  *   - "dev" pointers are CUDA device pointers on the device that was current
  *     at nb_create(); "host" pointers are ordinary host memory.
  *   - The CALLER owns every device byte (state, output, workspace).  The
- *     library owns only the host-side nb_ctx and never allocates device memory.
+ *     library owns only the host-side nb_ctx (plus one internal stream and two events) and
+ *     never allocates device memory.
  *     Borrowed pointers must stay valid until the next nb_set_state()/nb_destroy().
- *   - All device work is enqueued on the borrowed stream given to nb_create().
+ *   - All device work is ordered on the borrowed stream given to nb_create() (the contact
+ *     pass runs on a library-owned non-blocking stream, forked from and joined back into the
+ *     borrowed stream by events inside each force evaluation -- invisible to the caller).
  *     Nothing synchronises except nb_set_state(), nb_energy() and
  *     nb_download_state().  One ctx per host thread.
  *   - Element layout: elements of star 0 first, then star 1.  posm[i] =

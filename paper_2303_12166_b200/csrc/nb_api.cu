@@ -36,6 +36,8 @@ constexpr int kCtasPerSM = 8;                      // resident CTAs/SM of nb_gra
 constexpr int64_t kMaxSplit = 64;
 constexpr int64_t kPartialBudget = (int64_t)128 << 20;   // bytes of split-j partial sums worth keeping in L2
 constexpr int64_t kSortMinN = 8192;                // below this the contact pass takes groups in index order
+constexpr int64_t kContactWarps = 4096;            // warps wanted in flight by the contact kernel
+constexpr int kMaxContactChunks = 32;              // ... and splits the candidate groups of a warp into this many slabs
 
 // Force-path selection (nb_set_force_path).
 enum { kPathAuto = 0, kPathOneSided = 1, kPathSymmetric = 2 };
@@ -54,6 +56,19 @@ int sym_tile(int64_t n)
 
 int64_t sym_slabs(int64_t n) { const int64_t S = sym_tile(n); return (n + S - 1) / S; }
 
+// Slabs the contact pass writes for n elements: one per chunk of candidate groups (index order,
+// n < kSortMinN) or per round-robin share of the candidate groups (sorted search) that a warp takes.
+int contact_slabs(int64_t n)
+{
+    const int64_t ngroups = (n + kGroup - 1) / kGroup;
+    if (n < kSortMinN) return (int)(ngroups < kMaxContactChunks ? ngroups : kMaxContactChunks);
+    const int64_t nsuper = (ngroups + kSuper - 1) / kSuper;
+    int64_t ch = kContactWarps / ngroups;          // enough warps to fill the machine
+    if (ch > nsuper) ch = nsuper;
+    if (ch > kMaxContactChunks) ch = kMaxContactChunks;
+    return (int)(ch < 1 ? 1 : ch);
+}
+
 // Largest number of j splits allowed for n elements (bounds the partial-sum slabs).
 int64_t max_split(int64_t n)
 {
@@ -67,7 +82,7 @@ int64_t max_split(int64_t n)
 // grows with n, so the value for n_max covers every n <= n_max.
 int64_t partial_elems_bound(int64_t n_max)
 {
-    const int64_t a = (kMaxSplit + 1) * n_max;
+    const int64_t a = (kMaxSplit + kMaxContactChunks) * n_max;
     const int64_t b1 = 9 * n_max, b2 = kPartialBudget / 16 + n_max;
     const int64_t b = b1 > b2 ? b1 : b2;
     int64_t r = a < b ? a : b;
@@ -77,7 +92,7 @@ int64_t partial_elems_bound(int64_t n_max)
     int64_t probes[4] = {top, top, top, top};
     for (int k = 0; k < 3; ++k) if (tops[k] < top) probes[k + 1] = tops[k];
     for (int64_t n : probes) {
-        const int64_t e = (sym_slabs(n) + 1) * n;
+        const int64_t e = (sym_slabs(n) + contact_slabs(n)) * n;
         if (e > r) r = e;
     }
     return r;
@@ -151,6 +166,8 @@ struct nb_ctx {
     int64_t n_max = 0, n = 0;
     int n1 = 0;
     cudaStream_t stream = nullptr;
+    cudaStream_t side = nullptr;          // library-owned: the contact pass runs here, beside the gravity kernel
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int num_sms = kNumSMsFallback;
     float4* posm = nullptr;
     float4* vel = nullptr;
@@ -175,7 +192,11 @@ struct nb_ctx {
     float4* boxes() const { return reinterpret_cast<float4*>(ws + lay.off_boxes); }
     bool contact_on() const { return prm.gamma > 0.f; }
     int ngrav() const { return plan.sym_S ? plan.T : plan.nsplit; }       // gravity slabs
-    int nslabs() const { return ngrav() + (contact_on() ? 1 : 0); }       // slabs nb_reduce_update_kernel sums
+    int ncontact() const {                                                // contact slabs
+        if (!contact_on()) return 0;
+        return contact_slabs(n);
+    }
+    int nslabs() const { return ngrav() + ncontact(); }                   // slabs nb_reduce_update_kernel sums
 };
 
 #define NB_CUDA(ctx, call)                                   \
@@ -243,26 +264,26 @@ int launch_gravity(nb_ctx* c)
 }
 
 // Row a3: contact accelerations (Eqs. 5/6) of the pairs with r < R_i + R_j -> part[P][n]
-int launch_contact(nb_ctx* c)
+int launch_contact_on(nb_ctx* c, cudaStream_t st)
 {
     const int n = (int)c->n;
     const uint32_t* perm = nullptr;
     if (c->n >= kSortMinN) {
-        nb_bbox_kernel<<<kBoxBlocks, 256, 0, c->stream>>>(c->posm, n, c->boxes());
+        nb_bbox_kernel<<<kBoxBlocks, 256, 0, st>>>(c->posm, n, c->boxes());
         c->launches++;
-        nb_keys_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->posm, n, c->boxes(), c->keys(), c->vals());
+        nb_keys_kernel<<<(n + 255) / 256, 256, 0, st>>>(c->posm, n, c->boxes(), c->keys(), c->vals());
         c->launches++;
         NB_CUDA(c, cudaGetLastError());
         cub::DoubleBuffer<unsigned long long> dk(c->keys(), c->keys() + c->n_max);
         cub::DoubleBuffer<uint32_t> dv(c->vals(), c->vals() + c->n_max);
         size_t tmp = c->lay.sorttmp_bytes;
-        NB_CUDA(c, cub::DeviceRadixSort::SortPairs(c->ws + c->lay.off_sorttmp, tmp, dk, dv, n, 0, 3 * kKeyBits, c->stream));
+        NB_CUDA(c, cub::DeviceRadixSort::SortPairs(c->ws + c->lay.off_sorttmp, tmp, dk, dv, n, 0, 3 * kKeyBits, st));
         c->launches += 1;                              // counted as one (library) launch
         perm = dv.Current();
     }
     const int ngroups = (n + kGroup - 1) / kGroup;
     const int nsuper = (ngroups + kSuper - 1) / kSuper;
-    nb_gather_kernel<<<nsuper, kGroup * kSuper, 0, c->stream>>>(c->posm, c->vel, perm, n, c->dev(), c->ps(), c->vs(),
+    nb_gather_kernel<<<nsuper, kGroup * kSuper, 0, st>>>(c->posm, c->vel, perm, n, c->dev(), c->ps(), c->vs(),
                                                                c->gbox(), c->sbox());
     c->launches++;
     ContactArgs ca;
@@ -271,21 +292,38 @@ int launch_contact(nb_ctx* c)
     ca.n = n; ca.ngroups = ngroups; ca.nsuper = nsuper;
     ca.gamma = c->prm.gamma; ca.gamma_beta = c->prm.gamma * c->prm.beta;
     ca.v_dead = c->prm.v_dead; ca.lens_mode = c->prm.lens_mode;
-    nb_contact_kernel<<<(ngroups * 32 + kThreads - 1) / kThreads, kThreads, 0, c->stream>>>(ca);
+    const int nchunks = c->ncontact();
+    const long long warps = (long long)ngroups * nchunks;
+    ca.nchunks = nchunks; ca.spc = (nsuper + nchunks - 1) / nchunks;
+    if (perm) {
+        nb_contact_kernel<<<(int)((warps * 32 + kThreads - 1) / kThreads), kThreads, 0, st>>>(ca);
+    } else {
+        const int cg = (ngroups + nchunks - 1) / nchunks;
+        nb_contact_chunk_kernel<<<(int)((warps * 32 + kThreads - 1) / kThreads), kThreads, 0, st>>>(ca, cg, nchunks);
+    }
     c->launches++;
     NB_CUDA(c, cudaGetLastError());
     return NB_OK;
 }
 
-// Rows a2 + a3: every slab nb_reduce_update_kernel sums for a(x).  The contact pass goes first:
-// it is short, and the gravity kernel's CTAs then fill the machine behind it.
+int launch_contact(nb_ctx* c) { return launch_contact_on(c, c->stream); }
+
+// Rows a2 + a3: every slab nb_reduce_update_kernel sums for a(x).  The two are independent (both
+// read the state, each writes its own slabs), so the contact pass -- seven short launches that
+// cannot fill the machine -- runs on the library's side stream beside the gravity kernel:
+// fork after whatever the ctx stream holds, join before the update kernel.
 int launch_force(nb_ctx* c)
 {
-    if (c->contact_on()) {
-        const int rc = launch_contact(c);
-        if (rc) return rc;
-    }
-    return launch_gravity(c);
+    if (!c->contact_on()) return launch_gravity(c);
+    NB_CUDA(c, cudaEventRecord(c->ev_fork, c->stream));
+    NB_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_fork, 0));
+    int rc = launch_contact_on(c, c->side);
+    if (rc) return rc;
+    NB_CUDA(c, cudaEventRecord(c->ev_join, c->side));
+    rc = launch_gravity(c);
+    if (rc) return rc;
+    NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
+    return NB_OK;
 }
 
 // Rows a4+a6+a5: reduce `nsrc` slabs of `src`, optionally store a, kick, drift, advance.
@@ -355,12 +393,20 @@ int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream
     c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     c->num_sms = sms > 0 ? sms : kNumSMsFallback;
     c->lay = make_layout(n_max);
+    int prio_lo = 0, prio_hi = 0;                  // high priority: its small CTAs go first as gravity CTAs retire
+    cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
+    if (cudaStreamCreateWithPriority(&c->side, cudaStreamNonBlocking, prio_hi) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+        nb_destroy(c);
+        return NB_ECUDA;
+    }
     // the symmetric kernel's shared memory is dynamic (112 KB at S = 4096)
     if (cudaFuncSetAttribute(NB_SYM_512, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 512) != cudaSuccess ||
         cudaFuncSetAttribute(NB_SYM_1024, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 1024) != cudaSuccess ||
         cudaFuncSetAttribute(NB_SYM_2048, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 2048) != cudaSuccess ||
         cudaFuncSetAttribute(NB_SYM_4096, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 4096) != cudaSuccess) {
-        delete c;
+        nb_destroy(c);
         return NB_ECUDA;
     }
     {   // the radix sort's scratch must fit the slice the layout reserves for it
@@ -369,7 +415,7 @@ int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream
         cub::DoubleBuffer<uint32_t> dv(nullptr, nullptr);
         if (cub::DeviceRadixSort::SortPairs(nullptr, need, dk, dv, (int)n_max, 0, 3 * kKeyBits, c->stream) != cudaSuccess ||
             need > c->lay.sorttmp_bytes) {
-            delete c;
+            nb_destroy(c);
             return NB_ENOMEM;
         }
     }
@@ -377,7 +423,14 @@ int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream
     return NB_OK;
 }
 
-void nb_destroy(nb_ctx* ctx) { delete ctx; }
+void nb_destroy(nb_ctx* ctx)
+{
+    if (!ctx) return;
+    if (ctx->side) { cudaStreamSynchronize(ctx->side); cudaStreamDestroy(ctx->side); }
+    if (ctx->ev_fork) cudaEventDestroy(ctx->ev_fork);
+    if (ctx->ev_join) cudaEventDestroy(ctx->ev_join);
+    delete ctx;
+}
 
 int nb_set_state(nb_ctx* c, int64_t n, float* posm, float* vel, const int32_t* star, void* workspace,
                  size_t workspace_bytes)
@@ -413,7 +466,7 @@ int nb_set_state(nb_ctx* c, int64_t n, float* posm, float* vel, const int32_t* s
     c->posm = reinterpret_cast<float4*>(posm);
     c->vel = reinterpret_cast<float4*>(vel);
     c->plan = make_plan(n, c->num_sms, c->path);
-    if ((int64_t)(c->ngrav() + 1) * n > partial_elems_bound(c->n_max)) return NB_ENOMEM;
+    if ((int64_t)c->nslabs() * n > partial_elems_bound(c->n_max)) return NB_ENOMEM;
     c->have_state = true;
     return NB_OK;
 }
@@ -566,7 +619,7 @@ int nb_set_force_path(nb_ctx* c, int path)
     if (c->have_state) {
         const Plan p = make_plan(c->n, c->num_sms, path);
         const int64_t ngrav = p.sym_S ? p.T : p.nsplit;
-        if ((ngrav + 1) * c->n > partial_elems_bound(c->n_max)) return NB_ENOMEM;
+        if ((ngrav + c->ncontact()) * c->n > partial_elems_bound(c->n_max)) return NB_ENOMEM;
         c->plan = p;
     }
     c->path = path;

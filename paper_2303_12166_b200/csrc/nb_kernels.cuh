@@ -665,8 +665,11 @@ struct ContactArgs {
     const uint32_t* __restrict__ perm; // [n] original index of sorted element k (nullptr: identity)
     const float4* __restrict__ gbox;   // [2*ngroups]
     const float4* __restrict__ sbox;   // [2*nsuper]
-    float4* __restrict__ out;          // [n] contact acceleration, ORIGINAL index order
+    float4* __restrict__ out;          // [nchunks][n] contact acceleration, ORIGINAL index order
     int n, ngroups, nsuper;
+    int nchunks, spc;                  // nb_contact_kernel: the candidate groups of a group of elements i are dealt
+                                       // round-robin to nchunks warps (neighbours are adjacent on the Hilbert curve, so
+                                       // a split by ranges would leave all the work with one warp); spc unused
     float gamma, gamma_beta;           // Eq. 5 / Eq. 6 strengths
     float v_dead;
     int lens_mode;
@@ -756,8 +759,11 @@ nb_contact_kernel(const __grid_constant__ ContactArgs a)
     __shared__ int cand_s[kThreads / 32][kCandCap];
     __shared__ float4 stage_s[kThreads / 32][kGroup];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    const int ig = (blockIdx.x * kThreads + threadIdx.x) >> 5;     // group of elements i of this warp
+    const int wid = (blockIdx.x * kThreads + threadIdx.x) >> 5;
+    const int ig = wid / a.nchunks, ch = wid - ig * a.nchunks;     // group of elements i, chunk of super-groups
     if (ig >= a.ngroups) return;
+    const int sb0 = 0, sb1 = a.nsuper;             // every chunk warp scans all boxes; the candidates are dealt round-robin
+    int tot = 0;                                    // candidate groups found so far (the same in every chunk warp)
     int* cand = cand_s[wib];
     float4* stage = stage_s[wib];
     const int k = ig * kGroup + lane;
@@ -769,9 +775,9 @@ nb_contact_kernel(const __grid_constant__ ContactArgs a)
     double ax = 0.0, ay = 0.0, az = 0.0;
     int cnt = 0;
 
-    for (int sb = 0; sb < a.nsuper; sb += 32) {
+    for (int sb = sb0; sb < sb1; sb += 32) {
         bool near = false;
-        if (sb + lane < a.nsuper) {
+        if (sb + lane < sb1) {
             const float4 lo = a.sbox[2 * (sb + lane)], hi = a.sbox[2 * (sb + lane) + 1];
             const float D = ilo.w + lo.w;
             near = box_gap2(ilo, ihi, lo, hi) <= D * D * kSlack;
@@ -787,6 +793,9 @@ nb_contact_kernel(const __grid_constant__ ContactArgs a)
                 const float D = ilo.w + lo.w;
                 gnear = box_gap2(ilo, ihi, lo, hi) <= D * D * kSlack;
             }
+            const unsigned fmask = __ballot_sync(0xffffffffu, gnear);
+            gnear = gnear && ((tot + __popc(fmask & ((1u << lane) - 1u))) % a.nchunks == ch);
+            tot += __popc(fmask);
             const unsigned gmask = __ballot_sync(0xffffffffu, gnear);
             const int m = __popc(gmask);
             if (cnt + m > kCandCap) {                               // flush the list before it overflows
@@ -803,8 +812,37 @@ nb_contact_kernel(const __grid_constant__ ContactArgs a)
     contact_candidates(a, cand, cnt, stage, pi, vi, valid, lane, ax, ay, az);
     if (valid) {
         const int dst = a.perm ? (int)a.perm[k] : k;
-        a.out[dst] = make_float4((float)ax, (float)ay, (float)az, 0.f);
+        a.out[(size_t)ch * a.n + dst] = make_float4((float)ax, (float)ay, (float)az, 0.f);
     }
+}
+
+// Small n (groups in index order, no sort: every group is a candidate of every other): the
+// search above would leave n/32 warps walking all n elements one after the other.  Here a warp
+// owns (group of 32 elements i, chunk of `cg` candidate groups) and writes its own slab
+// out[chunk][i]; the update kernel adds the slabs in chunk order.
+__global__ void __launch_bounds__(kThreads)
+nb_contact_chunk_kernel(const __grid_constant__ ContactArgs a, const int cg, const int nchunks)
+{
+    __shared__ int cand_s[kThreads / 32][kCandCap];
+    __shared__ float4 stage_s[kThreads / 32][kGroup];
+    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    const int wid = (blockIdx.x * kThreads + threadIdx.x) >> 5;
+    const int ig = wid / nchunks, ch = wid - ig * nchunks;
+    if (ig >= a.ngroups) return;
+    const int k = ig * kGroup + lane;
+    const bool valid = k < a.n;
+    const float4 pi = valid ? a.ps[k] : make_float4(kFarAway, kFarAway, kFarAway, 0.f);
+    const float4 vi = valid ? a.vs[k] : make_float4(0.f, 0.f, 0.f, 1.f);
+    const int g0 = ch * cg, g1 = min(g0 + cg, a.ngroups);
+    double ax = 0.0, ay = 0.0, az = 0.0;
+    for (int gb = g0; gb < g1; gb += kCandCap) {
+        const int cnt = min(kCandCap, g1 - gb);
+        __syncwarp();
+        for (int q = lane; q < cnt; q += 32) cand_s[wib][q] = gb + q;
+        __syncwarp();
+        contact_candidates(a, cand_s[wib], cnt, stage_s[wib], pi, vi, valid, lane, ax, ay, az);
+    }
+    if (valid) a.out[(size_t)ch * a.n + k] = make_float4((float)ax, (float)ay, (float)az, 0.f);
 }
 
 // ---------------------------------------------------------------------------

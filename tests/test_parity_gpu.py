@@ -534,3 +534,31 @@ def test_runs_on_a_side_stream(nb):
     assert torch.equal(s.posm, ref.posm)
     assert nb.nb_time_force_kernel(s.ctx, 2) > 0
     s.close(); ref.close()
+
+
+@pytest.mark.parametrize("idx,scale", [(1, 1.0), (3, 0.75)])
+def test_steps_can_be_captured_in_a_cuda_graph(nb, idx, scale):
+    """nb_step() enqueues kernels, events and nothing else (no host synchronisation, step count and radii
+    live on the device), so a sequence of steps can be captured once and replayed: the replays must
+    continue the run bit for bit.  Covers the one-sided kernel + index-order contact pass (config 1) and
+    the symmetric kernel + sorted contact pass on the side stream, with the radius ramp (config 3 at 49,152)."""
+    import torch
+    w = make_config(idx, scale=scale)
+    p = params_f32(w.params)
+    st = torch.cuda.Stream()
+    s = nb.Simulation(w.posm, w.vel, w.star, p, stream=st)
+    ref = nb.Simulation(w.posm, w.vel, w.star, p)
+    s.step(1); s.synchronize()                       # the cached acceleration exists before the capture
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(g, stream=st):
+        s.step(3)
+    st.synchronize()
+    x_before = s.posm.clone()
+    g.replay(); g.replay()
+    torch.cuda.synchronize()
+    assert not torch.equal(x_before, s.posm)         # the capture itself ran nothing; the replays did
+    ref.step(1); ref.step(3); ref.step(3); ref.synchronize()
+    assert torch.equal(s.posm, ref.posm) and torch.equal(s.vel, ref.vel)
+    assert nb.nb_get_step(s.ctx) == nb.nb_get_step(ref.ctx)
+    assert nb.nb_get_step(s.ctx)[0] == 7
+    s.close(); ref.close()
