@@ -163,3 +163,95 @@ class Sim:
                           C.byref(prm), _dp(self.acc), _dp(out))
         return dict(KE=out[0], Ug=out[1], Urep=out[2], E=out[3], P=out[4:7].copy(),
                     L=out[7:10].copy(), Fnet=out[10], step=self.n)
+
+
+# ---------------------------------------------------------------------------------------------
+# NEXT rows of SURVEY.md 8(f) -- plain numpy, fp64 (same rules: test infrastructure only).
+
+def _sim_relax(self, k: int, kappa: float) -> None:
+    """f2, star construction / relaxation (the elements are put together and the star
+    is left to settle; the paper gives no procedure -- DESIGN.md reading A17): k leapfrog steps, each
+    followed by v <- (1 - kappa dt) v, the factor clamped at 0."""
+    f = max(0.0, 1.0 - float(kappa) * float(self.params["dt"]))
+    for _ in range(int(k)):
+        self.step(1)
+        self.v *= f
+
+
+Sim.relax = _sim_relax
+
+TRANSFER_FIELDS = ("M0", "M1", "a", "d0", "rL0", "rL1", "Mcross0", "Mcross1", "Min0", "Min1", "Mout0", "Mout1")
+
+
+def transfer_diagnostics(pos, vel, mass, star, k: float = 0.6, band: float = 0.0) -> Dict[str, object]:
+    """f3, mass transfer through L1 (reading A18).
+
+    Centres X_s, V_s and masses M_s of the two stars by membership; separation a = |X_1 - X_0| and
+    unit vector e; the L1 plane at distance d0 from X_0 along e (force balance, l1_distance); the
+    lobe radii rL_s = a * Eq. 3 with the star's own mass in the numerator.  Per star s (o = other):
+      Mcross_s  mass of its elements on the far side of the L1 plane,
+      Min_s     mass of its elements inside the other star's lobe sphere |x - X_o| < rL_o,
+      Ldisk_s   their angular momentum about the other star, sum m (x - X_o) x (v - V_o),
+      Mout_s    mass of its elements outside both lobe spheres.
+    `band` > 0 also returns 'ambiguous': the mass of elements within `band` of any of the decision
+    surfaces (either answer is acceptable for them in a comparison)."""
+    x, v, m = _f64(pos, 3), _f64(vel, 3), _f64(mass)
+    st = np.asarray(star).astype(np.int64)
+    M = np.array([m[st == s].sum() for s in (0, 1)])
+    X = np.array([(m[st == s, None] * x[st == s]).sum(0) / M[s] if M[s] > 0 else np.zeros(3) for s in (0, 1)])
+    V = np.array([(m[st == s, None] * v[st == s]).sum(0) / M[s] if M[s] > 0 else np.zeros(3) for s in (0, 1)])
+    out: Dict[str, object] = dict(M0=M[0], M1=M[1], X=X, V=V)
+    if not (M[0] > 0 and M[1] > 0):
+        out.update(a=0.0, d0=0.0, rL0=0.0, rL1=0.0, Mcross0=0.0, Mcross1=0.0, Min0=0.0, Min1=0.0,
+                   Mout0=0.0, Mout1=0.0, Ldisk=np.zeros((2, 3)), ambiguous=0.0)
+        return out
+    d = X[1] - X[0]
+    a = float(np.sqrt(d @ d))
+    e = d / a
+    if M[1] <= M[0]:
+        d0 = a * l1_distance(M[1] / M[0])                 # star 0 is the primary m1 of PAPER.md:28
+    else:
+        d0 = a * (1.0 - l1_distance(M[0] / M[1]))
+    rL = np.array([a * roche_lobe_radius(M[0] / M[1], k), a * roche_lobe_radius(M[1] / M[0], k)])
+    u = (x - X[0]) @ e
+    r0 = np.linalg.norm(x - X[0], axis=1)
+    r1 = np.linalg.norm(x - X[1], axis=1)
+    rs = [r0, r1]
+    Mcross, Min, Mout, Ld = np.zeros(2), np.zeros(2), np.zeros(2), np.zeros((2, 3))
+    for s in (0, 1):
+        o = 1 - s
+        mine = st == s
+        crossed = (u > d0) if s == 0 else (u < d0)
+        Mcross[s] = m[mine & crossed].sum()
+        inside = mine & (rs[o] < rL[o])
+        Min[s] = m[inside].sum()
+        Ld[s] = (m[inside, None] * np.cross(x[inside] - X[o], v[inside] - V[o])).sum(0)
+        Mout[s] = m[mine & (r0 > rL[0]) & (r1 > rL[1])].sum()
+    amb = 0.0
+    if band > 0:
+        near = (np.abs(u - d0) < band) | (np.abs(r0 - rL[0]) < band) | (np.abs(r1 - rL[1]) < band)
+        amb = float(m[near].sum())
+    out.update(a=a, d0=d0, rL0=rL[0], rL1=rL[1], Mcross0=Mcross[0], Mcross1=Mcross[1], Min0=Min[0],
+               Min1=Min[1], Mout0=Mout[0], Mout1=Mout[1], Ldisk=Ld, ambiguous=amb)
+    return out
+
+
+def splat(pos, star, centre, half_width: float, axis_u: int, axis_v: int, W: int, H: int) -> np.ndarray:
+    """f4, headless point splat replacing the paper's OpenGL viewer (the paper states no
+    shader math -- DESIGN.md reading A19): orthographic projection on coordinate axes (axis_u, axis_v),
+    pixel (floor((x_u - c_u) s + W/2), floor((x_v - c_v) s + H/2)) with s = W / (2 half_width), all in
+    float32 with one rounding per operation (the pixel index is an integer decided by floating point:
+    both sides take it in the kernel's precision); image[star][py][px] counts the elements, uint32."""
+    p = np.asarray(pos)[:, :3].astype(np.float32)
+    st = np.asarray(star).astype(np.int64)
+    c = np.asarray(centre, dtype=np.float32)
+    s = np.float32(np.float32(W) / np.float32(np.float32(2.0) * np.float32(half_width)))
+    fu = (p[:, axis_u] - c[axis_u]).astype(np.float32) * s
+    fu = (fu.astype(np.float32) + np.float32(0.5 * W)).astype(np.float32)
+    fv = (p[:, axis_v] - c[axis_v]).astype(np.float32) * s
+    fv = (fv.astype(np.float32) + np.float32(0.5 * H)).astype(np.float32)
+    pu, pv = np.floor(fu), np.floor(fv)
+    ok = (pu >= 0) & (pu < W) & (pv >= 0) & (pv < H)
+    img = np.zeros((2, H, W), dtype=np.uint32)
+    np.add.at(img, (st[ok], pv[ok].astype(np.int64), pu[ok].astype(np.int64)), 1)
+    return img
