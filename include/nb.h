@@ -106,6 +106,37 @@ int nb_step(nb_ctx* ctx, int nsteps);
  * U_grav = -sum_{i<j} G m_i m_j/(r+eps); U_rep per A12.  Synchronises the stream. */
 int nb_energy(nb_ctx* ctx, double* out);
 
+/* ---- SURVEY.md 8(f) "next" rows: built on the same state, kernels and stream ---------------
+ *
+ * f2, star construction (elements are put together and "this technique was used to
+ * create a binary system"; no procedure is printed -- reading A17): nsteps leapfrog steps as in
+ * nb_step(), each followed by v <- max(0, 1 - kappa*dt) v, so a star (or the binary) settles
+ * into equilibrium.  kappa >= 0 [1/time]; kappa = 0 is nb_step() exactly.  The step count and the
+ * radius ramp advance as usual.  Asynchronous on the stream. */
+int nb_relax(nb_ctx* ctx, int nsteps, float kappa);
+
+/* f3, mass transfer through L1 (reading A18), written to HOST out[32]:
+ *   [0] M0 [1] M1   masses of the two stars by membership;  [18..23] centres X0, X1;  [24..29] V0, V1
+ *   [2] a = |X1 - X0|   [3] d0: distance of the L1 plane from X0 along e = (X1 - X0)/a
+ *   [4] rL0 [5] rL1   Roche-lobe radii, a * Eq. 3 (constant k_lobe: 0.6 standard, 0.69 as printed, A9)
+ *   [6] Mcross0 [7] Mcross1   mass of star s's elements beyond the L1 plane (on the other star's side)
+ *   [8] Min0 [9] Min1         ... inside the OTHER star's lobe sphere |x - X_o| < rL_o
+ *   [10] Mout0 [11] Mout1     ... outside both lobe spheres
+ *   [12..14] Ldisk0 [15..17] Ldisk1   angular momentum of the Min_s elements about the other star,
+ *                                     sum m (x - X_o) x (v - V_o)
+ *   [30] step count, [31] 0.
+ * All sums and decisions in fp64 on the fp32 state.  Synchronises the stream (twice). */
+int nb_transfer_diagnostics(nb_ctx* ctx, double k_lobe, double* out);
+
+/* f4, headless point splat in place of the paper's OpenGL viewer (reading A19):
+ * orthographic projection of the element positions on coordinate axes (axis_u, axis_v in {0,1,2},
+ * different), window centred at HOST centre[3] with half width half_width along u (square pixels
+ * of 2*half_width/W), pixel = floor((x - c) * W/(2*half_width) + W/2 resp. H/2) evaluated in
+ * float32 with one rounding per operation.  image: dev uint32[2][H][W], caller-owned, overwritten
+ * with the number of elements of each star per pixel (exact, integer atomics).  Asynchronous. */
+int nb_splat(nb_ctx* ctx, const float* centre, float half_width, int axis_u, int axis_v, int W, int H,
+             uint32_t* image);
+
 /* Current step count n and element radii R_s(n) (host outputs; either may be NULL).
  * Synchronises the stream. */
 int nb_get_step(nb_ctx* ctx, int64_t* step, float* R);

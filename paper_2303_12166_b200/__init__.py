@@ -19,7 +19,8 @@ NB_OK, NB_EINVAL, NB_ESTATE, NB_ECUDA, NB_ENOMEM, NB_EARCH = 0, -1, -2, -3, -4, 
 NB_PATH_AUTO, NB_PATH_ONE_SIDED, NB_PATH_SYMMETRIC = 0, 1, 2
 
 EXPORTS = ("nb_create", "nb_workspace_bytes", "nb_set_state", "nb_compute_accel", "nb_step",
-           "nb_energy", "nb_get_step", "nb_upload_state", "nb_download_state",
+           "nb_energy", "nb_relax", "nb_transfer_diagnostics", "nb_splat", "nb_get_step", "nb_upload_state",
+           "nb_download_state",
            "nb_get_launch_info", "nb_set_force_path", "nb_force_kernel_name", "nb_launch_count",
            "nb_time_force_kernel", "nb_time_contact_pass", "nb_destroy", "nb_strerror",
            "nb_last_cuda_error", "nb_roche_lobe_radius", "nb_l1_distance")
@@ -67,6 +68,12 @@ def lib() -> C.CDLL:
         L.nb_step.argtypes = [vp, C.c_int]
         L.nb_energy.restype = C.c_int
         L.nb_energy.argtypes = [vp, C.POINTER(C.c_double)]
+        L.nb_relax.restype = C.c_int
+        L.nb_relax.argtypes = [vp, C.c_int, C.c_float]
+        L.nb_transfer_diagnostics.restype = C.c_int
+        L.nb_transfer_diagnostics.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
+        L.nb_splat.restype = C.c_int
+        L.nb_splat.argtypes = [vp, C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int, C.c_int, C.c_int, vp]
         L.nb_get_step.restype = C.c_int
         L.nb_get_step.argtypes = [vp, C.POINTER(i64), C.POINTER(C.c_float)]
         L.nb_upload_state.restype = C.c_int
@@ -164,6 +171,26 @@ def nb_energy(ctx: int) -> Dict[str, object]:
     return dict(KE=v[0], Ug=v[1], Urep=v[2], E=v[3], P=v[4:7], L=v[7:10], Fnet=v[10], step=int(v[11]))
 
 
+def nb_relax(ctx: int, nsteps: int, kappa: float) -> None:
+    _check(lib().nb_relax(ctx, int(nsteps), float(kappa)), "nb_relax", ctx)
+
+
+def nb_transfer_diagnostics(ctx: int, k_lobe: float = 0.6) -> Dict[str, object]:
+    out = (C.c_double * 32)()
+    _check(lib().nb_transfer_diagnostics(ctx, float(k_lobe), out), "nb_transfer_diagnostics", ctx)
+    v = list(out)
+    return dict(M0=v[0], M1=v[1], a=v[2], d0=v[3], rL0=v[4], rL1=v[5], Mcross0=v[6], Mcross1=v[7],
+                Min0=v[8], Min1=v[9], Mout0=v[10], Mout1=v[11], Ldisk=[v[12:15], v[15:18]],
+                X=[v[18:21], v[21:24]], V=[v[24:27], v[27:30]], step=int(v[30]))
+
+
+def nb_splat(ctx: int, centre: Sequence[float], half_width: float, axis_u: int, axis_v: int, W: int, H: int,
+             image) -> None:
+    c3 = (C.c_float * 3)(*[float(x) for x in centre])
+    _check(lib().nb_splat(ctx, c3, float(half_width), int(axis_u), int(axis_v), int(W), int(H), _ptr(image)),
+           "nb_splat", ctx)
+
+
 def nb_get_step(ctx: int):
     step = C.c_int64()
     R = (C.c_float * 2)()
@@ -259,6 +286,18 @@ class Simulation:
 
     def energy(self) -> Dict[str, object]:
         return nb_energy(self.ctx)
+
+    def relax(self, nsteps: int, kappa: float) -> None:
+        nb_relax(self.ctx, nsteps, kappa)
+
+    def transfer_diagnostics(self, k_lobe: float = 0.6) -> Dict[str, object]:
+        return nb_transfer_diagnostics(self.ctx, k_lobe)
+
+    def splat(self, centre, half_width: float, axis_u: int = 0, axis_v: int = 1, W: int = 512, H: int = 512):
+        with self.torch.cuda.stream(self.stream):
+            img = self.torch.empty((2, H, W), dtype=self.torch.int32, device=self.device)
+        nb_splat(self.ctx, centre, half_width, axis_u, axis_v, W, H, img)
+        return img
 
     def synchronize(self) -> None:
         self.stream.synchronize()

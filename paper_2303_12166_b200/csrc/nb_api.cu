@@ -144,7 +144,7 @@ Layout make_layout(int64_t n_max)
     L.off_acc = o;  o += align_up((size_t)n_max * sizeof(float4));
     L.off_part = o; o += align_up((size_t)partial_elems_bound(n_max) * sizeof(float4));
     const size_t pot_blocks = (size_t)((n_max + kThreads - 1) / kThreads);
-    const size_t red = (size_t)kMomentBlocks * kMomentCols * sizeof(double) + pot_blocks * 2 * sizeof(double);
+    const size_t red = (size_t)kMomentBlocks * 16 * sizeof(double) + pot_blocks * 2 * sizeof(double);   // 16 >= kMomentCols, kXferCols1, kXferCols2
     L.off_red = o;  o += align_up(red);
     L.off_keys = o; o += align_up((size_t)n_max * 2 * sizeof(unsigned long long));   // key double buffer
     L.off_vals = o; o += align_up((size_t)n_max * 2 * sizeof(uint32_t));             // index double buffer
@@ -328,11 +328,11 @@ int launch_force(nb_ctx* c)
 
 // Rows a4+a6+a5: reduce `nsrc` slabs of `src`, optionally store a, kick, drift, advance.
 int launch_update(nb_ctx* c, const float4* src, int nsrc, float4* acc_out, float kick_h, float drift_dt,
-                  int advance)
+                  int advance, float vscale = 1.f)
 {
     UpdateArgs u;
     u.src = src; u.acc_out = acc_out; u.posm = c->posm; u.vel = c->vel; u.dev = c->dev();
-    u.n = (int)c->n; u.nsrc = nsrc; u.kick_h = kick_h; u.drift_dt = drift_dt; u.advance = advance;
+    u.n = (int)c->n; u.nsrc = nsrc; u.kick_h = kick_h; u.drift_dt = drift_dt; u.advance = advance; u.vscale = vscale;
     const int grid = (int)((c->n + 255) / 256);
     nb_reduce_update_kernel<<<grid, 256, 0, c->stream>>>(u);
     c->launches++;
@@ -508,6 +508,98 @@ int nb_step(nb_ctx* c, int nsteps)
         if (rc) return rc;
     }
     c->have_acc = true;
+    return NB_OK;
+}
+
+int nb_relax(nb_ctx* c, int nsteps, float kappa)
+{
+    if (!c || nsteps < 0 || !(kappa >= 0.f) || !std::isfinite(kappa)) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    if (nsteps == 0) return NB_OK;
+    const float dt = c->prm.dt;
+    float f = 1.f - kappa * dt;                               // rounded as written: one multiply, one subtract
+    if (!(f > 0.f)) f = 0.f;
+    int rc = ensure_acc(c);
+    if (rc) return rc;
+    for (int s = 0; s < nsteps; ++s) {
+        rc = launch_update(c, c->acc(), 1, nullptr, 0.5f * dt, dt, 1);          // half kick, drift, n += 1
+        if (rc) return rc;
+        rc = launch_force(c);
+        if (rc) return rc;
+        rc = launch_update(c, c->part(), c->nslabs(), c->acc(), 0.5f * dt, 0.f, 0, f);   // half kick, then v <- f v
+        if (rc) return rc;
+    }
+    c->have_acc = true;
+    return NB_OK;
+}
+
+int nb_transfer_diagnostics(nb_ctx* c, double k_lobe, double* out)
+{
+    if (!c || !out || !(k_lobe > 0.0) || !std::isfinite(k_lobe)) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    const int n = (int)c->n;
+    double* red = c->red();
+    double h1[kMomentBlocks * kXferCols1], h2[kMomentBlocks * kXferCols2];
+    nb_star_moments_kernel<<<kMomentBlocks, 256, 0, c->stream>>>(c->posm, c->vel, n, c->n1, red);
+    c->launches++;
+    NB_CUDA(c, cudaGetLastError());
+    DevState hs;
+    NB_CUDA(c, cudaMemcpyAsync(h1, red, sizeof(h1), cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaMemcpyAsync(&hs, c->dev(), sizeof(hs), cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    double q[kXferCols1] = {0};
+    for (int b = 0; b < kMomentBlocks; ++b)
+        for (int k = 0; k < kXferCols1; ++k) q[k] += h1[b * kXferCols1 + k];
+    for (int k = 0; k < 32; ++k) out[k] = 0.0;
+    const double M0 = q[0], M1 = q[7];
+    out[0] = M0; out[1] = M1; out[30] = (double)hs.step;
+    XferArgs xa;
+    for (int s = 0; s < 2; ++s) {
+        const double M = s ? M1 : M0;
+        for (int k = 0; k < 3; ++k) {
+            xa.X[s][k] = M > 0.0 ? q[7 * s + 1 + k] / M : 0.0;
+            xa.V[s][k] = M > 0.0 ? q[7 * s + 4 + k] / M : 0.0;
+            out[18 + 3 * s + k] = xa.X[s][k];
+            out[24 + 3 * s + k] = xa.V[s][k];
+        }
+    }
+    if (!(M0 > 0.0 && M1 > 0.0)) return NB_OK;                 // one star only: nothing to transfer
+    double d[3], a2 = 0.0;
+    for (int k = 0; k < 3; ++k) { d[k] = xa.X[1][k] - xa.X[0][k]; a2 += d[k] * d[k]; }
+    const double a = std::sqrt(a2);
+    if (!(a > 0.0)) return NB_OK;
+    for (int k = 0; k < 3; ++k) xa.e[k] = d[k] / a;
+    // L1 along the line of centres, measured from star 0 (nb_l1_distance is measured from the primary)
+    xa.d0 = M1 <= M0 ? a * nb_l1_distance(M1 / M0) : a * (1.0 - nb_l1_distance(M0 / M1));
+    xa.rL[0] = a * nb_roche_lobe_radius(M0 / M1, k_lobe);      // Eq. 3: the star's own mass in the numerator
+    xa.rL[1] = a * nb_roche_lobe_radius(M1 / M0, k_lobe);
+    xa.posm = c->posm; xa.vel = c->vel; xa.out = red; xa.n = n; xa.n1 = c->n1;
+    nb_transfer_kernel<<<kMomentBlocks, 256, 0, c->stream>>>(xa);
+    c->launches++;
+    NB_CUDA(c, cudaGetLastError());
+    NB_CUDA(c, cudaMemcpyAsync(h2, red, sizeof(h2), cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    double r[kXferCols2] = {0};
+    for (int b = 0; b < kMomentBlocks; ++b)
+        for (int k = 0; k < kXferCols2; ++k) r[k] += h2[b * kXferCols2 + k];
+    out[2] = a; out[3] = xa.d0; out[4] = xa.rL[0]; out[5] = xa.rL[1];
+    for (int k = 0; k < kXferCols2; ++k) out[6 + k] = r[k];    // Mcross[2], Min[2], Mout[2], Ldisk[2][3]
+    return NB_OK;
+}
+
+int nb_splat(nb_ctx* c, const float* centre, float half_width, int axis_u, int axis_v, int W, int H,
+             uint32_t* image)
+{
+    if (!c || !centre || !image || !(half_width > 0.f) || !std::isfinite(half_width)) return NB_EINVAL;
+    if (axis_u < 0 || axis_u > 2 || axis_v < 0 || axis_v > 2 || axis_u == axis_v) return NB_EINVAL;
+    if (W < 1 || H < 1 || W > 16384 || H > 16384 || ((uintptr_t)image & 3)) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    const float scale = (float)W / (2.0f * half_width);        // pixels per unit length, fp32
+    NB_CUDA(c, cudaMemsetAsync(image, 0, (size_t)2 * W * H * sizeof(uint32_t), c->stream));
+    nb_splat_kernel<<<(int)((c->n + 255) / 256), 256, 0, c->stream>>>(c->posm, (int)c->n, c->n1, centre[axis_u],
+                                                                     centre[axis_v], scale, axis_u, axis_v, W, H, image);
+    c->launches++;
+    NB_CUDA(c, cudaGetLastError());
     return NB_OK;
 }
 

@@ -859,6 +859,7 @@ struct UpdateArgs {
     DevState* dev;
     int n, nsrc;
     float kick_h, drift_dt;
+    float vscale;                      // relaxation (f2): v <- vscale (v + kick_h a); 1 for the plain leapfrog
     int advance;
 };
 
@@ -874,11 +875,12 @@ nb_reduce_update_kernel(const __grid_constant__ UpdateArgs u)
         }
         const float ax = (float)sx, ay = (float)sy, az = (float)sz;
         if (u.acc_out) u.acc_out[i] = make_float4(ax, ay, az, 0.f);
-        if (u.kick_h != 0.f || u.drift_dt != 0.f) {
+        if (u.kick_h != 0.f || u.drift_dt != 0.f || u.vscale != 1.f) {
             float4 v = u.vel[i];
             v.x = fmaf(u.kick_h, ax, v.x);
             v.y = fmaf(u.kick_h, ay, v.y);
             v.z = fmaf(u.kick_h, az, v.z);
+            if (u.vscale != 1.f) { v.x *= u.vscale; v.y *= u.vscale; v.z *= u.vscale; }
             u.vel[i] = v;
             if (u.drift_dt != 0.f) {
                 float4 p = u.posm[i];
@@ -1017,6 +1019,94 @@ nb_potential_kernel(const __grid_constant__ PotArgs a)
     const double e1 = block_sum((double)a.G * (double)pi.w * phi, sh);
     const double e2 = block_sum(i < a.n ? urep : 0.0, sh);
     if (tid == 0) { a.out[2 * (size_t)blockIdx.x] = e1; a.out[2 * (size_t)blockIdx.x + 1] = e2; }
+}
+
+// ---------------------------------------------------------------------------
+// Row f3: mass transfer through L1 (A18).
+// Pass 1: per star (by membership: star 0 = indices < n1) M, sum m x, sum m v -- block partials.
+constexpr int kXferCols1 = 14;        // per star: M, Mx, My, Mz, Mvx, Mvy, Mvz
+constexpr int kXferCols2 = 12;        // Mcross[2], Min[2], Mout[2], Ldisk[2][3]
+
+__global__ void __launch_bounds__(256)
+nb_star_moments_kernel(const float4* __restrict__ posm, const float4* __restrict__ vel, int n, int n1,
+                       double* __restrict__ out /*[grid][14]*/)
+{
+    __shared__ double sh[8];
+    double q[kXferCols1];
+    for (int c = 0; c < kXferCols1; ++c) q[c] = 0.0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const float4 p = posm[i], v = vel[i];
+        const double m = p.w;
+        double* t = q + (i < n1 ? 0 : 7);
+        t[0] += m;
+        t[1] += m * (double)p.x; t[2] += m * (double)p.y; t[3] += m * (double)p.z;
+        t[4] += m * (double)v.x; t[5] += m * (double)v.y; t[6] += m * (double)v.z;
+    }
+    for (int c = 0; c < kXferCols1; ++c) {
+        const double r = block_sum(q[c], sh);
+        if (threadIdx.x == 0) out[(size_t)blockIdx.x * kXferCols1 + c] = r;
+    }
+}
+
+// Pass 2: every decision in fp64 on the fp32 coordinates.
+struct XferArgs {
+    const float4* __restrict__ posm;
+    const float4* __restrict__ vel;
+    double* __restrict__ out;          // [grid][12]
+    int n, n1;
+    double X[2][3], V[2][3], e[3], d0, rL[2];
+};
+
+__global__ void __launch_bounds__(256)
+nb_transfer_kernel(const __grid_constant__ XferArgs a)
+{
+    __shared__ double sh[8];
+    double q[kXferCols2];
+    for (int c = 0; c < kXferCols2; ++c) q[c] = 0.0;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += gridDim.x * blockDim.x) {
+        const float4 p = a.posm[i], v = a.vel[i];
+        const int s = i < a.n1 ? 0 : 1, o = 1 - s;
+        const double m = p.w;
+        const double x0 = (double)p.x - a.X[0][0], y0 = (double)p.y - a.X[0][1], z0 = (double)p.z - a.X[0][2];
+        const double x1 = (double)p.x - a.X[1][0], y1 = (double)p.y - a.X[1][1], z1 = (double)p.z - a.X[1][2];
+        const double u = x0 * a.e[0] + y0 * a.e[1] + z0 * a.e[2];
+        const double r0 = sqrt(x0 * x0 + y0 * y0 + z0 * z0), r1 = sqrt(x1 * x1 + y1 * y1 + z1 * z1);
+        if (s == 0 ? (u > a.d0) : (u < a.d0)) q[s] += m;                       // beyond the L1 plane
+        if ((o == 0 ? r0 : r1) < a.rL[o]) {                                    // inside the other star's lobe sphere
+            q[2 + s] += m;
+            const double rx = o == 0 ? x0 : x1, ry = o == 0 ? y0 : y1, rz = o == 0 ? z0 : z1;
+            const double wx = (double)v.x - a.V[o][0], wy = (double)v.y - a.V[o][1], wz = (double)v.z - a.V[o][2];
+            q[6 + 3 * s] += m * (ry * wz - rz * wy);
+            q[7 + 3 * s] += m * (rz * wx - rx * wz);
+            q[8 + 3 * s] += m * (rx * wy - ry * wx);
+        }
+        if (r0 > a.rL[0] && r1 > a.rL[1]) q[4 + s] += m;                       // outside both
+    }
+    for (int c = 0; c < kXferCols2; ++c) {
+        const double r = block_sum(q[c], sh);
+        if (threadIdx.x == 0) a.out[(size_t)blockIdx.x * kXferCols2 + c] = r;
+    }
+}
+
+// ---------------------------------------------------------------------------
+// Row f4: headless point splat in place of the paper's OpenGL viewer
+// (A19).  Orthographic projection on two coordinate axes; the pixel index
+// is decided in float32 with one rounding per operation (no FMA contraction), the same
+// arithmetic the oracle spells out; counts are integer atomics, so the image is exact.
+__global__ void __launch_bounds__(256)
+nb_splat_kernel(const float4* __restrict__ posm, int n, int n1, float cu, float cv, float scale,
+                int axis_u, int axis_v, int W, int H, unsigned int* __restrict__ image /*[2][H][W]*/)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float4 p = posm[i];
+    const float xu = axis_u == 0 ? p.x : (axis_u == 1 ? p.y : p.z);
+    const float xv = axis_v == 0 ? p.x : (axis_v == 1 ? p.y : p.z);
+    const float fu = floorf(__fadd_rn(__fmul_rn(__fsub_rn(xu, cu), scale), 0.5f * (float)W));
+    const float fv = floorf(__fadd_rn(__fmul_rn(__fsub_rn(xv, cv), scale), 0.5f * (float)H));
+    if (!(fu >= 0.f && fu < (float)W && fv >= 0.f && fv < (float)H)) return;
+    const int s = i < n1 ? 0 : 1;
+    atomicAdd(&image[((size_t)s * H + (int)fv) * W + (int)fu], 1u);
 }
 
 }  // namespace nb

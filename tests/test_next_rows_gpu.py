@@ -1,0 +1,220 @@
+"""GPU parity of the SURVEY.md 8(f) "next" rows, through the C ABI, against the oracle:
+f1 scenario variants (parameter sets of the same kernels), f2 relaxation steps, f3 mass-transfer
+diagnostics, f4 point splat."""
+import numpy as np
+import pytest
+
+import oracle
+from workloads import make_config, make_scenario, params_f32, SCENARIOS
+
+pytestmark = pytest.mark.gpu
+
+POS_TOL = 1.0e-4
+ACC_TOL = 2.0e-5
+
+
+def _sim(nb, w, p=None, **kw):
+    return nb.Simulation(w.posm, w.vel, w.star, p or params_f32(w.params), **kw)
+
+
+# ------------------------------------------------------------------ f1: scenarios
+@pytest.mark.parametrize("key", sorted(SCENARIOS))
+def test_scenario_accel_and_ten_steps(nb, key):
+    """Each of the paper's three kinds of run: accelerations and a 10-step
+    trajectory, with the per-star radius ramps (both stars expanding in case B)."""
+    w = make_scenario(key)
+    p = params_f32(w.params)
+    s = _sim(nb, w, p)
+    a = s.compute_accel().cpu().numpy().astype(np.float64)[:, :3]
+    a_or, kap, dl = oracle.accel(w.posm, w.vel, w.posm[:, 3], w.star, p["R_start"], p, want_diag=True)
+    err = np.linalg.norm(a - a_or, axis=1)
+    an = np.linalg.norm(a_or, axis=1)
+    assert (np.maximum(err - dl, 0) / an).max() <= ACC_TOL
+    s.step(10); s.synchronize()
+    o = oracle.Sim(w.posm, w.vel, w.star, p); o.step(10)
+    x = s.posm.cpu().numpy().astype(np.float64)[:, :3]
+    step, R = nb.nb_get_step(s.ctx)
+    assert step == 10 and np.array_equal(np.asarray(R, np.float64), o.radii().astype(np.float32).astype(np.float64))
+    if key == "case_b_both_expand":
+        assert R[0] > p["R_start"][0] and R[1] > p["R_start"][1]
+    assert np.linalg.norm(x - o.x, axis=1).max() / w.meta["a"] <= POS_TOL
+    s.close()
+
+
+def test_scenario_long_run_invariants_and_transfer_begins(nb):
+    """Case B at a quarter of its size, the full 200-step ramp: momentum and angular momentum conserved,
+    no NaN, and the expanding stars start to push elements across the L1 plane."""
+    w = make_scenario("case_b_both_expand", scale=0.25)
+    s = _sim(nb, w)
+    e0, t0 = s.energy(), s.transfer_diagnostics()
+    s.step(200)
+    e1, t1 = s.energy(), s.transfer_diagnostics()
+    assert t1["step"] == 200 and np.isfinite([e1["E"], e1["KE"]]).all()
+    Lz = abs(e0["L"][2])
+    assert np.abs(np.array(e1["P"]) - np.array(e0["P"])).max() < 1e-5 * 0.3
+    assert np.abs(np.array(e1["L"]) - np.array(e0["L"])).max() < 1e-4 * Lz
+    assert t1["M0"] == pytest.approx(t0["M0"], rel=1e-12) and t1["M1"] == pytest.approx(t0["M1"], rel=1e-12)
+    assert t1["Mcross0"] + t1["Mcross1"] >= t0["Mcross0"] + t0["Mcross1"]
+    s.close()
+
+
+# ------------------------------------------------------------------ f2: relaxation
+@pytest.mark.parametrize("kappa", [0.0, 5.0, 40.0, 5000.0])
+def test_relax_parity(nb, kappa):
+    w = make_config(1)
+    p = params_f32(w.params)
+    s = _sim(nb, w, p)
+    s.relax(10, kappa); s.synchronize()
+    o = oracle.Sim(w.posm, w.vel, w.star, p); o.relax(10, kappa)
+    x = s.posm.cpu().numpy().astype(np.float64)[:, :3]
+    v = s.vel.cpu().numpy().astype(np.float64)[:, :3]
+    assert np.linalg.norm(x - o.x, axis=1).max() / w.meta["a"] <= POS_TOL
+    assert np.linalg.norm(v - o.v, axis=1).max() / (w.meta["omega"] * w.meta["a"]) <= 1e-2
+    if kappa * p["dt"] >= 1.0:
+        assert (v == 0).all()
+    assert nb.nb_get_step(s.ctx)[0] == 10
+    s.close()
+
+
+def test_relax_zero_damping_is_nb_step_bitwise_and_mixes_with_it(nb):
+    import torch
+    w = make_config(3, scale=0.75)                  # symmetric kernel + radius ramp
+    p = params_f32(w.params)
+    a, b = _sim(nb, w, p), _sim(nb, w, p)
+    a.relax(3, 0.0); a.step(2); b.step(5)
+    a.synchronize(); b.synchronize()
+    # relax() splits the two half kicks that step() merges (v + h a + h a vs v + 2h a): same to rounding
+    assert torch.allclose(a.posm, b.posm, rtol=0, atol=2e-6) and torch.allclose(a.vel, b.vel, rtol=0, atol=2e-6)
+    assert nb.nb_get_step(a.ctx) == nb.nb_get_step(b.ctx)
+    a.close(); b.close()
+
+
+def test_relax_settles_a_single_star(nb):
+    """One star alone (a star is put together from elements first): damping drains the
+    kinetic energy the Poisson-random placement releases; momentum stays ~0; the star stays bound."""
+    w = make_config(1)
+    n1 = w.meta["n1"]
+    posm, vel, star = w.posm[:n1].copy(), np.zeros_like(w.vel[:n1]), w.star[:n1].copy()
+    p = params_f32(dict(w.params, dt=2e-3))
+    s = nb.Simulation(posm, vel, star, p)
+    s.relax(150, 0.0)
+    hot = s.energy()
+    s.relax(300, 25.0)
+    cold = s.energy()
+    assert cold["KE"] < 0.2 * hot["KE"] and cold["E"] < hot["E"]
+    assert np.abs(cold["P"]).max() < 1e-5
+    x = s.posm.cpu().numpy()[:, :3].astype(np.float64)
+    r = np.linalg.norm(x - x.mean(0), axis=1)
+    assert np.isfinite(r).all() and np.median(r) < 1.5
+    s.close()
+
+
+def test_relax_argument_errors(nb):
+    s = _sim(nb, make_config(1, scale=0.125))
+    L = nb.lib()
+    assert L.nb_relax(s.ctx, -1, 0.0) == nb.NB_EINVAL
+    assert L.nb_relax(s.ctx, 1, -0.5) == nb.NB_EINVAL
+    assert L.nb_relax(s.ctx, 1, float("nan")) == nb.NB_EINVAL
+    assert L.nb_relax(None, 1, 0.0) == nb.NB_EINVAL
+    assert L.nb_relax(s.ctx, 0, 1.0) == nb.NB_OK
+    s.close()
+
+
+# ------------------------------------------------------------------ f3: transfer diagnostics
+def _check_transfer(nb, posm, vel, star, p, k=0.6):
+    s = nb.Simulation(posm, vel, star, p)
+    g = s.transfer_diagnostics(k)
+    s.close()
+    o = oracle.transfer_diagnostics(posm, vel, posm[:, 3], star, k, band=1e-9)
+    for f in ("M0", "M1", "a", "d0", "rL0", "rL1"):
+        assert g[f] == pytest.approx(o[f], rel=1e-12), f
+    assert np.allclose(g["X"], o["X"], rtol=0, atol=1e-12) and np.allclose(g["V"], o["V"], rtol=0, atol=1e-12)
+    slack = o["ambiguous"] + 1e-12 * (o["M0"] + o["M1"])       # elements sitting on a decision surface
+    for f in ("Mcross0", "Mcross1", "Min0", "Min1", "Mout0", "Mout1"):
+        assert abs(g[f] - o[f]) <= slack, (f, g[f], o[f])
+    Lscale = max(np.abs(o["Ldisk"]).max(), 1e-300)
+    assert np.abs(np.array(g["Ldisk"]) - o["Ldisk"]).max() <= 1e-11 * Lscale + slack * 10
+    return g, o
+
+
+@pytest.mark.parametrize("idx", [1, 3])
+def test_transfer_diagnostics_parity_detached(nb, idx):
+    w = make_config(idx)
+    g, _ = _check_transfer(nb, w.posm, w.vel, w.star, params_f32(w.params))
+    assert g["Mcross0"] == g["Min0"] == 0.0 and g["step"] == 0
+
+
+@pytest.mark.parametrize("k", [0.6, 0.69])
+def test_transfer_diagnostics_parity_with_transferred_mass(nb, k):
+    """Config 3 with a twentieth of the donor displaced toward and past the accretor: every output
+    is non-trivial (elements beyond L1, inside the accretor's lobe with angular momentum, and outside)."""
+    w = make_config(3)
+    rng = np.random.default_rng(5)
+    m = w.n // 20
+    w.posm[:m, :3] += np.float32([1.3, 0.05, 0.0]) + rng.normal(0, 0.4, (m, 3)).astype(np.float32)
+    w.posm[m:2 * m, 2] += np.float32(3.0)            # a puff far above the plane: outside both lobes
+    g, o = _check_transfer(nb, w.posm, w.vel, w.star, params_f32(w.params), k)
+    assert g["Mcross0"] > 0.01 and g["Min0"] > 0.001 and g["Mout0"] > 0.01 and abs(g["Ldisk"][0][2]) > 0
+
+
+def test_transfer_diagnostics_heavier_second_star_and_single_star(nb):
+    w = make_config(1)
+    w.posm[w.star == 1, 3] *= np.float32(4.0)        # star 1 becomes the primary: mirrored L1
+    g, o = _check_transfer(nb, w.posm, w.vel, w.star, params_f32(w.params))
+    assert g["M1"] > g["M0"] and g["d0"] < 0.5 * g["a"]
+    n1 = w.meta["n1"]
+    s = nb.Simulation(w.posm[:n1].copy(), w.vel[:n1].copy(), w.star[:n1].copy(), params_f32(w.params))
+    g1 = s.transfer_diagnostics()
+    s.close()
+    assert g1["M1"] == 0.0 and g1["a"] == 0.0 and g1["Mcross0"] == 0.0
+    assert g1["M0"] == pytest.approx(float(w.posm[:n1, 3].astype(np.float64).sum()), rel=1e-12)
+
+
+def test_transfer_diagnostics_argument_errors(nb):
+    import ctypes as C
+    s = _sim(nb, make_config(1, scale=0.125))
+    out = (C.c_double * 32)()
+    L = nb.lib()
+    assert L.nb_transfer_diagnostics(s.ctx, 0.0, out) == nb.NB_EINVAL
+    assert L.nb_transfer_diagnostics(s.ctx, 0.6, None) == nb.NB_EINVAL
+    assert L.nb_transfer_diagnostics(None, 0.6, out) == nb.NB_EINVAL
+    s.close()
+
+
+# ------------------------------------------------------------------ f4: point splat
+@pytest.mark.parametrize("axes,W,H,hw", [((0, 1), 256, 256, 3.0), ((0, 2), 640, 360, 2.5), ((2, 1), 33, 77, 0.7)])
+def test_splat_is_bit_exact(nb, axes, W, H, hw):
+    w = make_config(3)
+    s = _sim(nb, w)
+    centre = [0.4, -0.1, 0.05]
+    img = s.splat(centre, hw, axes[0], axes[1], W, H)
+    s.synchronize()
+    ref = oracle.splat(w.posm, w.star, centre, hw, axes[0], axes[1], W, H)
+    got = img.cpu().numpy().astype(np.int64)
+    assert got.shape == ref.shape and np.array_equal(got, ref.astype(np.int64))
+    if hw >= 2.5:
+        assert got.sum() > 0.9 * w.n
+    s.step(2)                                        # the image follows the state
+    img2 = s.splat(centre, hw, axes[0], axes[1], W, H)
+    s.synchronize()
+    x = s.posm.cpu().numpy()
+    assert np.array_equal(img2.cpu().numpy().astype(np.int64),
+                          oracle.splat(x, w.star, centre, hw, axes[0], axes[1], W, H).astype(np.int64))
+    s.close()
+
+
+def test_splat_argument_errors(nb):
+    import torch
+    import ctypes as C
+    s = _sim(nb, make_config(1, scale=0.125))
+    img = torch.zeros((2, 8, 8), dtype=torch.int32, device="cuda")
+    c3 = (C.c_float * 3)(0, 0, 0)
+    L = nb.lib()
+    assert L.nb_splat(s.ctx, c3, 1.0, 0, 0, 8, 8, img.data_ptr()) == nb.NB_EINVAL      # same axis twice
+    assert L.nb_splat(s.ctx, c3, 0.0, 0, 1, 8, 8, img.data_ptr()) == nb.NB_EINVAL
+    assert L.nb_splat(s.ctx, c3, 1.0, 0, 3, 8, 8, img.data_ptr()) == nb.NB_EINVAL
+    assert L.nb_splat(s.ctx, c3, 1.0, 0, 1, 0, 8, img.data_ptr()) == nb.NB_EINVAL
+    assert L.nb_splat(s.ctx, None, 1.0, 0, 1, 8, 8, img.data_ptr()) == nb.NB_EINVAL
+    assert L.nb_splat(s.ctx, c3, 1.0, 0, 1, 8, 8, None) == nb.NB_EINVAL
+    assert L.nb_splat(s.ctx, c3, 1.0, 0, 1, 8, 8, img.data_ptr()) == nb.NB_OK
+    s.close()

@@ -5,4 +5,5 @@ no Roche formula): only the recipes that lay out two stars of elements, as
 DESIGN.md "Input recipe" states them.  Both the CUDA path and the CPU oracle
 consume the float32 arrays produced here.
 """
-from .configs import CONFIGS, make_config, make_binary, params_f32, Workload  # noqa: F401
+from .configs import (CONFIGS, SCENARIOS, make_config, make_binary, make_scenario, params_f32,  # noqa: F401
+                      Workload)

@@ -70,7 +70,7 @@ def make_binary(*, name: str, seed: int, n1: int, n2: int, shape: str,
                 radius1: float, radius2: float, q: float, a: float, eps: float,
                 dt: float, nsteps: int, mass_sigma: float = 0.0,
                 noise_frac: float = NOISE_FRAC, ramp_factor1: float = 1.0,
-                n_ramp: int = 0, gamma: float = GAMMA, beta: float = BETA,
+                ramp_factor2: float = 1.0, n_ramp: int = 0, gamma: float = GAMMA, beta: float = BETA,
                 G: float = 1.0) -> Workload:
     """Two stars of elements on a circular orbit with synchronous rotation.
 
@@ -113,7 +113,7 @@ def make_binary(*, name: str, seed: int, n1: int, n2: int, shape: str,
     re2 = radius2 * (PHI_PACK / max(n2, 1)) ** (1.0 / 3.0)
     vscale = math.sqrt(G * (M1 + M2) / a)
     params = dict(G=G, eps=eps, dt=dt, q=q, gamma=gamma, beta=beta,
-                  R_start=(re1, re2), R_end=(re1 * ramp_factor1, re2),
+                  R_start=(re1, re2), R_end=(re1 * ramp_factor1, re2 * ramp_factor2),
                   n_ramp=int(n_ramp), v_dead=V_DEAD_FRAC * vscale,
                   tau_s=TAU_S_FRAC * vscale, lens_mode=0)
     meta = dict(a=a, omega=omega, n1=n1, n2=n2, nsteps=nsteps, seed=seed,
@@ -164,3 +164,29 @@ def params_f32(params: Dict[str, object]) -> Dict[str, object]:
         if k in out:
             out[k] = tuple(f(v) for v in out[k])
     return out
+
+
+# the paper's three kinds of run (Fig. 5), as parameter sets of the
+# same recipe.  The paper prints no numbers for them; sizes are kept small enough for a full oracle run.
+SCENARIOS = {
+    # I-III: main-sequence donor filling its lobe + compact accretor (white dwarf): few, small elements
+    "ms_white_dwarf": dict(name="scenario_ms_white_dwarf", seed=11, n1=16384, n2=1024, shape="uniform",
+                           radius1=1.0, radius2=0.08, q=0.6, a=2.6, eps=0.004, dt=5e-4, nsteps=200,
+                           ramp_factor1=1.12, n_ramp=200),
+    # IV-VI: non-conservative case B, two main-sequence stars, BOTH expanding
+    "case_b_both_expand": dict(name="scenario_case_b", seed=12, n1=8192, n2=8192, shape="uniform",
+                               radius1=1.0, radius2=0.9, q=0.8, a=2.4, eps=0.005, dt=5e-4, nsteps=200,
+                               ramp_factor1=1.2, ramp_factor2=1.2, n_ramp=200),
+    # VII-IX: red giant (large, tenuous) + main-sequence star, Algol-like
+    "algol_red_giant": dict(name="scenario_algol", seed=13, n1=12288, n2=8192, shape="uniform",
+                            radius1=1.5, radius2=0.5, q=0.5, a=3.4, eps=0.005, dt=1e-3, nsteps=200,
+                            ramp_factor1=1.1, n_ramp=100),
+}
+
+
+def make_scenario(key: str, scale: Optional[float] = None) -> Workload:
+    kw = dict(SCENARIOS[key])
+    if scale is not None:
+        kw["n1"] = max(1, int(round(kw["n1"] * scale)))
+        kw["n2"] = max(1, int(round(kw["n2"] * scale)))
+    return make_binary(**kw)
