@@ -64,9 +64,15 @@ __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
     f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
 }
 
-// add2 that the compiler may neither move nor fold (see sym_sweep).
+// Packed operations that the compiler may neither reorder among themselves nor fold (see sym_step, sym_sweep).
 __device__ __forceinline__ f32x2 add2v(f32x2 a, f32x2 b) {
     f32x2 d; asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
+}
+__device__ __forceinline__ f32x2 fma2v(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 d; asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d;
+}
+__device__ __forceinline__ f32x2 mul2v(f32x2 a, f32x2 b) {
+    f32x2 d; asm volatile("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
 }
 
 // Radius of the star an element index belongs to (star 0 first, then star 1).
@@ -319,6 +325,26 @@ __device__ __forceinline__ void sym_step(const float4 p0, const float4 p1,
             ci0 = mul2(c0, pk2(p0.w, p0.w)); ci1 = mul2(c1, pk2(p1.w, p1.w));   // G m_j for a_i
             if (SYM) { cj0 = mul2(c0, gmi[h]); cj1 = mul2(c1, gmi[h]); }        // G m_i for a_j
         }
+        if (SYM && JP && UNI) {
+            // a_i and the reaction use the same (c, d): issued back to back, the second instruction takes
+            // both from the operand reuse cache and reads only its accumulator from the register file
+            if (h == 0) {
+                ax[h] = fma2v(c0, dx0, ax[h]); ga[0] = mul2v(c0, dx0);
+                ay[h] = fma2v(c0, dy0, ay[h]); ga[1] = mul2v(c0, dy0);
+                az[h] = fma2v(c0, dz0, az[h]); ga[2] = mul2v(c0, dz0);
+                ax[h] = fma2v(c1, dx1, ax[h]); gb[0] = mul2v(c1, dx1);
+                ay[h] = fma2v(c1, dy1, ay[h]); gb[1] = mul2v(c1, dy1);
+                az[h] = fma2v(c1, dz1, az[h]); gb[2] = mul2v(c1, dz1);
+            } else {
+                ax[h] = fma2v(c0, dx0, ax[h]); ga[0] = fma2v(c0, dx0, ga[0]);
+                ay[h] = fma2v(c0, dy0, ay[h]); ga[1] = fma2v(c0, dy0, ga[1]);
+                az[h] = fma2v(c0, dz0, az[h]); ga[2] = fma2v(c0, dz0, ga[2]);
+                ax[h] = fma2v(c1, dx1, ax[h]); gb[0] = fma2v(c1, dx1, gb[0]);
+                ay[h] = fma2v(c1, dy1, ay[h]); gb[1] = fma2v(c1, dy1, gb[1]);
+                az[h] = fma2v(c1, dz1, az[h]); gb[2] = fma2v(c1, dz1, gb[2]);
+            }
+            continue;
+        }
         ax[h] = fma2(ci0, dx0, ax[h]); ay[h] = fma2(ci0, dy0, ay[h]); az[h] = fma2(ci0, dz0, az[h]);
         ax[h] = fma2(ci1, dx1, ax[h]); ay[h] = fma2(ci1, dy1, ay[h]); az[h] = fma2(ci1, dz1, az[h]);
         if (SYM && !JP) {                                                  // reaction: a_j -= [G m_i] c d
@@ -354,7 +380,7 @@ __device__ __forceinline__ void sym_step(const float4 p0, const float4 p1,
 
 // All tiles of super-tile B (in shared memory) against the warp's 64 H elements i, for every
 // round of elements i of super-tile A.
-template <int S, int H, int NT, bool JP, bool MONT, bool UNI, bool SYM>
+template <int S, int H, int NT, bool JP, bool MONT, int UNR, bool UNI, bool SYM>
 __device__ __forceinline__ void sym_sweep(const SymArgs& a, const int A, const int B, const float4* __restrict__ jpos,
                                           float* __restrict__ jax, float* __restrict__ jay, float* __restrict__ jaz,
                                           const double scale_i)
@@ -398,7 +424,7 @@ __device__ __forceinline__ void sym_sweep(const SymArgs& a, const int A, const i
 #pragma unroll
             for (int h = 0; h < H; ++h) ax[h] = ay[h] = az[h] = pk2(0.f, 0.f);
             float ja[3] = {0.f, 0.f, 0.f}, jb[3] = {0.f, 0.f, 0.f};
-#pragma unroll 2
+#pragma unroll UNR
             for (int k = 0; k < 32; ++k) {
                 const int slot = (lane + k) & 31;
                 sym_step<H, UNI, SYM, JP, MONT>(tp[slot], tp[32 + slot], nxi, nyi, nzi, gmi, eps2, ax, ay, az, ja, jb);
@@ -434,7 +460,7 @@ __device__ __forceinline__ void sym_sweep(const SymArgs& a, const int A, const i
     }
 }
 
-template <int S, int H, int NT, int MINB, bool JP, bool MONT>
+template <int S, int H, int NT, int MINB, bool JP, bool MONT, int UNR = 2>
 __global__ void __launch_bounds__(NT, MINB)
 nb_gravity_sym_kernel(const __grid_constant__ SymArgs a)
 {
@@ -476,12 +502,12 @@ nb_gravity_sym_kernel(const __grid_constant__ SymArgs a)
     const int uni = __syncthreads_and(u ? 1 : 0);
 
     if (A == B) {
-        if (uni) sym_sweep<S, H, NT, JP, MONT, true, false>(a, A, B, jpos, jax, jay, jaz, (double)(a.G * mB));
-        else     sym_sweep<S, H, NT, JP, MONT, false, false>(a, A, B, jpos, jax, jay, jaz, 1.0);
+        if (uni) sym_sweep<S, H, NT, JP, MONT, UNR, true, false>(a, A, B, jpos, jax, jay, jaz, (double)(a.G * mB));
+        else     sym_sweep<S, H, NT, JP, MONT, UNR, false, false>(a, A, B, jpos, jax, jay, jaz, 1.0);
         return;
     }
-    if (uni) sym_sweep<S, H, NT, JP, MONT, true, true>(a, A, B, jpos, jax, jay, jaz, (double)(a.G * mB));
-    else     sym_sweep<S, H, NT, JP, MONT, false, true>(a, A, B, jpos, jax, jay, jaz, 1.0);
+    if (uni) sym_sweep<S, H, NT, JP, MONT, UNR, true, true>(a, A, B, jpos, jax, jay, jaz, (double)(a.G * mB));
+    else     sym_sweep<S, H, NT, JP, MONT, UNR, false, true>(a, A, B, jpos, jax, jay, jaz, 1.0);
 
     // reaction sums of super-tile B due to super-tile A (sign: a_j -= ...)
     const double scale_j = uni ? -(double)(a.G * mA) : -1.0;
