@@ -253,11 +253,11 @@ def run_own(args):
     step_ms = ms_total / args.steps
     # What the kernel executes per ordered interaction (FMA-pipe flop + one per MUFU), as opposed to the
     # 21 flop Eq. 4 itself needs (the convention `achieved` uses).  One-sided kernel: 20.5 + 1.5 (Montgomery
-    # costs 1.5 more multiplies and saves half a MUFU).  Symmetric kernel: one pair evaluation of 26.5 + 1.5
-    # serves two interactions (the super-tiles on the diagonal run one-sided: weight S/N).
+    # costs 1.5 more multiplies and saves half a MUFU).  Symmetric kernel: one pair evaluation of 25 + 2
+    # serves two interactions (the super-tiles on the diagonal run one-sided, 19 + 2 each: weight S/N).
     if symmetric:
         diag = info["i_per_cta"] / float(n)
-        executed = (1.0 - diag) * 14.0 + diag * 22.0
+        executed = (1.0 - diag) * 13.5 + diag * 21.0
     else:
         executed = 22.0
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
