@@ -260,18 +260,23 @@ nb_gravity_kernel(const __grid_constant__ GravArgs a)
 // Eq. 4 is a force "between elements i and j": F_ij = -F_ji, so the geometric
 // factor c = 1/(r (r+eps)^2) and the difference d of a pair serve both a_i += G m_j c d and
 // a_j -= G m_i c d.  Elements are cut into super-tiles of S; one CTA owns one pair of
-// super-tiles (A <= B).  Its 8 warps each keep 64 elements i of A in registers (two per lane, one
-// packed pair) and walk the tiles of 64 elements j of B.  Inside a tile the warp ROTATES: at step
-// k lane l meets slots (l+k)&31 and 32+((l+k)&31) (conflict-free LDS.128), accumulates a_i in its
-// own registers and the pair's reaction in six scalar registers that travel with the slots
-// (SHFL to lane l-1 after every step); after 32 steps the lane holds the finished sums of slots l
-// and 32+l over the warp's 64 elements i and adds them to the CTA's shared-memory array.  The
-// warps of a CTA are skewed over different tiles and meet at a barrier after every tile, so the
-// shared-memory sums have a fixed order: results are bitwise reproducible.
-// Per lane and step (2 i x 2 j = 4 pairs = 8 interactions): the 27 packed instructions of the
-// one-sided loop (FADD2 x6, FFMA2 x6+2, FMUL2 x9, FFMA2 x6 -- see above) give c and a_i, 12 scalar FFMA
-// add the reaction, 6 SHFL rotate it: 39 FMA-pipe instructions per 8 interactions instead of
-// 54, and 0.75 MUFU per interaction instead of 1.5.
+// super-tiles (A <= B).  Each of its NT/32 warps keeps 64 H elements i of A in registers (2 H per
+// lane: H packed pairs) and walks the tiles of 64 elements j of B.  Inside a tile the warp
+// ROTATES: at step k lane l meets slots (l+k)&31 and 32+((l+k)&31) (conflict-free LDS.128),
+// accumulates a_i in its own registers and the pairs' reaction in six scalar registers that travel
+// with the slots (SHFL to lane l-1 after every step); after 32 steps the lane holds the finished
+// sums of slots l and 32+l over the warp's 64 H elements i and adds them to the CTA's shared-memory
+// array.  The warps of a CTA are skewed over different tiles and meet at a barrier after every
+// tile, so the shared-memory sums have a fixed order: results are bitwise reproducible.
+// Template parameters: S super-tile, H packed pairs of i per lane, NT threads, MINB CTAs/SM,
+//   JP    reaction summed in packed form (FMUL2/FFMA2 issued right behind the a_i FFMA2 of the same
+//         (c, d): both sources come from the operand reuse cache) and folded by two FADD, instead of
+//         one scalar FFMA per pair;
+//   MONT  reciprocal shared by the two j of a lane (as in the one-sided kernel) instead of one
+//         MUFU.RCP per pair;   UNR  unroll of the 32-step rotation.
+// Shipped: H = 2, JP, no MONT, UNR = 4 (DESIGN.md 5.1c lists what the others measured).  Per lane
+// and step (4 i x 2 j = 8 pairs = 16 interactions): 48 + 12 packed FP32 instructions, 12 FADD,
+// 16 MUFU, 6 SHFL, 2 LDS.128 -- 13.5 executed flop per interaction against 22 one-sided.
 // Output: part[Y][e] = acceleration of element e due to the elements of super-tile Y (every
 // (Y, tile of e) combination is written by exactly one CTA; the diagonal CTAs (A == B) run the
 // one-sided loop).  Super-tiles of one mass take the mass out of the loop, as in
