@@ -160,7 +160,7 @@ int nb_download_state(nb_ctx* ctx, float* host_posm, float* host_vel, float* hos
 int nb_get_launch_info(nb_ctx* ctx, int32_t* out4);
 
 /* Which kernel evaluates row a2 (Eq. 4, summed over all pairs).
- *   NB_PATH_AUTO (default): the symmetric kernel for 32768 <= n <= 2097152, else the one-sided
+ *   NB_PATH_AUTO (default): the symmetric kernel for 24576 <= n <= 2097152, else the one-sided
  *     kernel (the symmetric kernel is never used above 2097152 elements: its partial sums would
  *     not fit; NB_PATH_SYMMETRIC then falls back to the one-sided kernel as well).
  *   NB_PATH_ONE_SIDED: every ORDERED pair (i, j) is evaluated; a CTA owns an (i-block, j-split).
@@ -169,8 +169,7 @@ int nb_get_launch_info(nb_ctx* ctx, int32_t* out4);
  *     super-tiles.  Both compute the same sum in a fixed order (bitwise reproducible run to run);
  *     they differ from each other by fp32 rounding only.
  * May be called before or after nb_set_state(); NB_ENOMEM if the bound workspace cannot hold the
- * partial sums of the requested path for the bound n (it always can for n_max >= 32768 or the
- * default path).  Drops nothing: the cached acceleration stays valid. */
+ * partial sums of the requested path for the bound n (it always can for the default path).  Drops nothing: the cached acceleration stays valid. */
 enum { NB_PATH_AUTO = 0, NB_PATH_ONE_SIDED = 1, NB_PATH_SYMMETRIC = 2 };
 int nb_set_force_path(nb_ctx* ctx, int path);
 

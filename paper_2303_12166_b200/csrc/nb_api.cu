@@ -41,13 +41,17 @@ constexpr int kMaxContactChunks = 32;              // ... and splits the candida
 
 // Force-path selection (nb_set_force_path).
 enum { kPathAuto = 0, kPathOneSided = 1, kPathSymmetric = 2 };
-constexpr int64_t kSymMinN = 32768;               // auto: symmetric kernel from here on (enough CTAs to fill the SMs)
+constexpr int64_t kSymMinN = 24576;               // auto: symmetric kernel from here on.  The kernel alone wins from ~6,000
+                                                  // elements, but its 126 registers leave the contact pass no room to run
+                                                  // beside it: whole steps are equal at 16,384 and 10 % shorter at 24,576
+constexpr int64_t kSym256MaxN = 32768;             // below this the super-tiles are 256 elements (CTAs of 2 warps)
 constexpr int64_t kSymMaxN = (int64_t)1 << 21;    // ... up to here: its T slabs of n float4 reach 17 GB at 2M elements
 
 // Super-tile size of the symmetric kernel for n elements: its T = ceil(n/S) slabs of n float4
 // partial sums cost memory and one extra pass, so S grows with n.
 int sym_tile(int64_t n)
 {
+    if (n < kSym256MaxN) return 256;  // small n: more, smaller CTAs
     if (n < 98304) return 512;        // T <= 192
     if (n < 196608) return 1024;      // T <= 192
     if (n < 786432) return 2048;      // T <= 384
@@ -88,9 +92,9 @@ int64_t partial_elems_bound(int64_t n_max)
     int64_t r = a < b ? a : b;
     // symmetric kernel: (T(n) + 1) n, largest just below each change of the super-tile size
     const int64_t top = n_max < kSymMaxN ? n_max : kSymMaxN;
-    const int64_t tops[3] = {98303, 196607, 786431};
-    int64_t probes[4] = {top, top, top, top};
-    for (int k = 0; k < 3; ++k) if (tops[k] < top) probes[k + 1] = tops[k];
+    const int64_t tops[4] = {kSym256MaxN - 1, 98303, 196607, 786431};
+    int64_t probes[5] = {top, top, top, top, top};
+    for (int k = 0; k < 4; ++k) if (tops[k] < top) probes[k + 1] = tops[k];
     for (int64_t n : probes) {
         const int64_t e = (sym_slabs(n) + contact_slabs(n)) * n;
         if (e > r) r = e;
@@ -226,6 +230,7 @@ bool params_ok(const nb_params* p)
 }
 
 // The instantiations of the symmetric kernel: <S, H, threads, CTAs/SM, packed reaction, Montgomery, unroll>.
+#define NB_SYM_256  nb_gravity_sym_kernel<256, 2, 64, 8, true, false, 4>
 #define NB_SYM_512  nb_gravity_sym_kernel<512, 2, 128, 4, true, false, 4>
 #define NB_SYM_1024 nb_gravity_sym_kernel<1024, 2, 256, 2, true, false, 4>
 #define NB_SYM_2048 nb_gravity_sym_kernel<2048, 2, 256, 2, true, false, 4>
@@ -243,7 +248,8 @@ int launch_gravity(nb_ctx* c)
         const long long T = c->plan.T;
         const int grid = (int)(T * (T + 1) / 2);
         const int smem = kSymSmemPerElem * c->plan.sym_S;
-        if (c->plan.sym_S == 512)       NB_SYM_512<<<grid, 128, smem, c->stream>>>(sa);
+        if (c->plan.sym_S == 256)       NB_SYM_256<<<grid, 64, smem, c->stream>>>(sa);
+        else if (c->plan.sym_S == 512)  NB_SYM_512<<<grid, 128, smem, c->stream>>>(sa);
         else if (c->plan.sym_S == 1024) NB_SYM_1024<<<grid, 256, smem, c->stream>>>(sa);
         else if (c->plan.sym_S == 2048) NB_SYM_2048<<<grid, 256, smem, c->stream>>>(sa);
         else                            NB_SYM_4096<<<grid, 256, smem, c->stream>>>(sa);
@@ -721,6 +727,7 @@ int nb_set_force_path(nb_ctx* c, int path)
 const char* nb_force_kernel_name(nb_ctx* c)
 {
     if (!c || !c->have_state) return "";
+    if (c->plan.sym_S == 256) return "nb_gravity_sym_kernel<256,2,64,8,1,0,4>";
     if (c->plan.sym_S == 512) return "nb_gravity_sym_kernel<512,2,128,4,1,0,4>";
     if (c->plan.sym_S == 1024) return "nb_gravity_sym_kernel<1024,2,256,2,1,0,4>";
     if (c->plan.sym_S == 2048) return "nb_gravity_sym_kernel<2048,2,256,2,1,0,4>";

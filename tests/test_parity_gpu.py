@@ -112,9 +112,11 @@ def test_symmetric_path_full_parity_ragged_sizes(nb, n1, n2):
 
 
 @pytest.mark.parametrize("idx", [1, 2])
-def test_symmetric_path_small_configs(nb, idx):
-    """Config 2 has lognormal masses: every super-tile takes the per-pair mass multiplies."""
-    _check_accel(nb, make_config(idx), force_path=nb.NB_PATH_SYMMETRIC)
+@pytest.mark.parametrize("path", [1, 2])
+def test_both_paths_small_configs(nb, idx, path):
+    """Configs 1 and 2 by each kernel (the default is one-sided for both).  Config 2 has
+    lognormal masses: every tile / super-tile takes the per-pair mass multiplies."""
+    _check_accel(nb, make_config(idx), force_path=path)
 
 
 @pytest.mark.parametrize("override", [dict(gamma=0.0), dict(eps=0.0), dict(G=0.0), dict(G=2.5, eps=0.05)])
@@ -153,9 +155,9 @@ def test_default_path_and_both_paths_agree_at_full_size(nb):
     _check_accel(nb, w, p, rows=_sample(w.n, 1024, 5), force_path=nb.NB_PATH_ONE_SIDED)
 
 
-@pytest.mark.parametrize("n,name", [(32768, "<512"), (120000, "<1024"), (400000, "<2048")])
+@pytest.mark.parametrize("n,name", [(24576, "<256"), (30001, "<256"), (32768, "<512"), (120000, "<1024"), (400000, "<2048")])
 def test_symmetric_tile_bands(nb, n, name):
-    """One size in each super-tile band below config 5's (S = 512, 1024, 2048; 4096 is config 5),
+    """Sizes in each super-tile band below config 5's (S = 256, 512, 1024, 2048; 4096 is config 5),
     ragged against the band's tile, sampled rows against the oracle."""
     w = _ragged(n - n // 3, n // 3, seed=21, eps=0.004)
     p = params_f32(w.params)
