@@ -755,12 +755,34 @@ __device__ __forceinline__ float point_gap2(const float4 p, const float4 lo, con
 }
 
 constexpr int kCandCap = 128;         // candidate groups buffered per warp before they are processed
+constexpr int kHitCap = 40;           // per-lane queue of pairs that passed the fp32 pre-test (a group adds <= 32)
+constexpr int kHitFlush = 8;          // the queues are drained once any lane holds this many
 
-// Evaluate the lane's element i against the `cnt` candidate groups listed in cand[]:
+// Drain the warp's hit queues: every lane evaluates ITS OWN queued pairs in the order it found them
+// (so the fp64 sums have the same fixed order as an immediate evaluation would give), all lanes in
+// step -- the fp64 contact term is ~80 instructions, and evaluated at the point of discovery it ran
+// with one or two lanes active.
+__device__ __forceinline__ void contact_drain(const ContactArgs& a, const uint32_t* __restrict__ hq, int& nh,
+                                              const float4 pi, const float4 vi, int lane,
+                                              double& ax, double& ay, double& az)
+{
+    const int mx = __reduce_max_sync(0xffffffffu, nh);
+    for (int k = 0; k < mx; ++k) {
+        if (k < nh) {
+            const int j = (int)hq[k * 32 + lane];
+            contact_term(a, pi, vi, a.ps[j], a.vs[j], ax, ay, az);
+        }
+    }
+    nh = 0;
+}
+
+// Test the lane's element i against the `cnt` candidate groups listed in cand[]:
 // a group is skipped unless some lane's point is within reach of its box; its 32 elements are
-// staged in the warp's shared-memory slot (coalesced load, broadcast reads).
+// staged in the warp's shared-memory slot (coalesced load, broadcast reads); pairs that pass the
+// fp32 pre-test go to the lane's hit queue.
 __device__ __forceinline__ void contact_candidates(const ContactArgs& a, const int* __restrict__ cand, int cnt,
-                                                   float4* __restrict__ stage, const float4 pi, const float4 vi,
+                                                   float4* __restrict__ stage, uint32_t* __restrict__ hq, int& nh,
+                                                   const float4 pi, const float4 vi,
                                                    bool valid, int lane, double& ax, double& ay, double& az)
 {
     const float kSlack = 1.0f + 1.0e-5f;
@@ -779,8 +801,9 @@ __device__ __forceinline__ void contact_candidates(const ContactArgs& a, const i
             const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
             const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
             const float D = pi.w + pj.w;
-            if (r2 <= D * D * kSlack && valid) contact_term(a, pi, vi, pj, a.vs[j0 + t], ax, ay, az);
+            if (r2 <= D * D * kSlack && valid) { hq[nh * 32 + lane] = (uint32_t)(j0 + t); ++nh; }
         }
+        if (__any_sync(0xffffffffu, nh >= kHitFlush)) contact_drain(a, hq, nh, pi, vi, lane, ax, ay, az);
     }
 }
 
@@ -789,7 +812,10 @@ nb_contact_kernel(const __grid_constant__ ContactArgs a)
 {
     __shared__ int cand_s[kThreads / 32][kCandCap];
     __shared__ float4 stage_s[kThreads / 32][kGroup];
+    __shared__ uint32_t hit_s[kThreads / 32][kHitCap * 32];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    uint32_t* hq = hit_s[wib];
+    int nh = 0;
     const int wid = (blockIdx.x * kThreads + threadIdx.x) >> 5;
     const int ig = wid / a.nchunks, ch = wid - ig * a.nchunks;     // group of elements i, chunk of super-groups
     if (ig >= a.ngroups) return;
@@ -831,7 +857,7 @@ nb_contact_kernel(const __grid_constant__ ContactArgs a)
             const int m = __popc(gmask);
             if (cnt + m > kCandCap) {                               // flush the list before it overflows
                 __syncwarp();
-                contact_candidates(a, cand, cnt, stage, pi, vi, valid, lane, ax, ay, az);
+                contact_candidates(a, cand, cnt, stage, hq, nh, pi, vi, valid, lane, ax, ay, az);
                 cnt = 0;
                 __syncwarp();
             }
@@ -840,7 +866,8 @@ nb_contact_kernel(const __grid_constant__ ContactArgs a)
         }
     }
     __syncwarp();
-    contact_candidates(a, cand, cnt, stage, pi, vi, valid, lane, ax, ay, az);
+    contact_candidates(a, cand, cnt, stage, hq, nh, pi, vi, valid, lane, ax, ay, az);
+    contact_drain(a, hq, nh, pi, vi, lane, ax, ay, az);
     if (valid) {
         const int dst = a.perm ? (int)a.perm[k] : k;
         a.out[(size_t)ch * a.n + dst] = make_float4((float)ax, (float)ay, (float)az, 0.f);
@@ -856,7 +883,10 @@ nb_contact_chunk_kernel(const __grid_constant__ ContactArgs a, const int cg, con
 {
     __shared__ int cand_s[kThreads / 32][kCandCap];
     __shared__ float4 stage_s[kThreads / 32][kGroup];
+    __shared__ uint32_t hit_s[kThreads / 32][kHitCap * 32];
     const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+    uint32_t* hq = hit_s[wib];
+    int nh = 0;
     const int wid = (blockIdx.x * kThreads + threadIdx.x) >> 5;
     const int ig = wid / nchunks, ch = wid - ig * nchunks;
     if (ig >= a.ngroups) return;
@@ -871,8 +901,9 @@ nb_contact_chunk_kernel(const __grid_constant__ ContactArgs a, const int cg, con
         __syncwarp();
         for (int q = lane; q < cnt; q += 32) cand_s[wib][q] = gb + q;
         __syncwarp();
-        contact_candidates(a, cand_s[wib], cnt, stage_s[wib], pi, vi, valid, lane, ax, ay, az);
+        contact_candidates(a, cand_s[wib], cnt, stage_s[wib], hq, nh, pi, vi, valid, lane, ax, ay, az);
     }
+    contact_drain(a, hq, nh, pi, vi, lane, ax, ay, az);
     if (valid) a.out[(size_t)ch * a.n + k] = make_float4((float)ax, (float)ay, (float)az, 0.f);
 }
 
