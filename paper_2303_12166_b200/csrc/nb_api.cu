@@ -51,9 +51,9 @@ constexpr int64_t kSymMaxN = (int64_t)1 << 21;    // ... up to here: its T slabs
 // partial sums cost memory and one extra pass, so S grows with n.
 int sym_tile(int64_t n)
 {
-    if (n < kSym256MaxN) return 256;  // small n: more, smaller CTAs
+    if (n < kSym256MaxN) return 256;  // small n: more, smaller CTAs (T <= 128)
     if (n < 98304) return 512;        // T <= 192
-    if (n < 196608) return 1024;      // T <= 192
+    if (n < 393216) return 1024;      // T <= 384
     if (n < 786432) return 2048;      // T <= 384
     return 4096;
 }
@@ -92,7 +92,7 @@ int64_t partial_elems_bound(int64_t n_max)
     int64_t r = a < b ? a : b;
     // symmetric kernel: (T(n) + 1) n, largest just below each change of the super-tile size
     const int64_t top = n_max < kSymMaxN ? n_max : kSymMaxN;
-    const int64_t tops[4] = {kSym256MaxN - 1, 98303, 196607, 786431};
+    const int64_t tops[4] = {kSym256MaxN - 1, 98303, 393215, 786431};
     int64_t probes[5] = {top, top, top, top, top};
     for (int k = 0; k < 4; ++k) if (tops[k] < top) probes[k + 1] = tops[k];
     for (int64_t n : probes) {
@@ -229,12 +229,12 @@ bool params_ok(const nb_params* p)
     return true;
 }
 
-// The instantiations of the symmetric kernel: <S, H, threads, CTAs/SM, packed reaction, Montgomery, unroll>.
-#define NB_SYM_256  nb_gravity_sym_kernel<256, 2, 64, 8, true, false, 4>
-#define NB_SYM_512  nb_gravity_sym_kernel<512, 2, 128, 4, true, false, 4>
-#define NB_SYM_1024 nb_gravity_sym_kernel<1024, 2, 256, 2, true, false, 4>
-#define NB_SYM_2048 nb_gravity_sym_kernel<2048, 2, 256, 2, true, false, 4>
-#define NB_SYM_4096 nb_gravity_sym_kernel<4096, 2, 256, 2, true, false, 4>
+// The instantiations of the symmetric kernel: <S, elements i per lane, threads, CTAs/SM, unroll>.
+#define NB_SYM_256  nb_gravity_sym_kernel<256, 4, 64, 8, 4>
+#define NB_SYM_512  nb_gravity_sym_kernel<512, 4, 128, 4, 4>
+#define NB_SYM_1024 nb_gravity_sym_kernel<1024, 4, 256, 2, 4>
+#define NB_SYM_2048 nb_gravity_sym_kernel<2048, 4, 256, 2, 4>
+#define NB_SYM_4096 nb_gravity_sym_kernel<4096, 4, 256, 2, 4>
 
 // Row a2: partial gravitational accelerations -> part[0..ngrav-1][n]
 //   symmetric kernel: one CTA per pair of super-tiles, part[Y][e] = a_e due to super-tile Y
@@ -727,11 +727,11 @@ int nb_set_force_path(nb_ctx* c, int path)
 const char* nb_force_kernel_name(nb_ctx* c)
 {
     if (!c || !c->have_state) return "";
-    if (c->plan.sym_S == 256) return "nb_gravity_sym_kernel<256,2,64,8,1,0,4>";
-    if (c->plan.sym_S == 512) return "nb_gravity_sym_kernel<512,2,128,4,1,0,4>";
-    if (c->plan.sym_S == 1024) return "nb_gravity_sym_kernel<1024,2,256,2,1,0,4>";
-    if (c->plan.sym_S == 2048) return "nb_gravity_sym_kernel<2048,2,256,2,1,0,4>";
-    if (c->plan.sym_S) return "nb_gravity_sym_kernel<4096,2,256,2,1,0,4>";
+    if (c->plan.sym_S == 256) return "nb_gravity_sym_kernel<256,4,64,8,4>";
+    if (c->plan.sym_S == 512) return "nb_gravity_sym_kernel<512,4,128,4,4>";
+    if (c->plan.sym_S == 1024) return "nb_gravity_sym_kernel<1024,4,256,2,4>";
+    if (c->plan.sym_S == 2048) return "nb_gravity_sym_kernel<2048,4,256,2,4>";
+    if (c->plan.sym_S) return "nb_gravity_sym_kernel<4096,4,256,2,4>";
     return c->plan.TJ == 256 ? "nb_gravity_kernel<2,256>" : "nb_gravity_kernel<2,128>";
 }
 

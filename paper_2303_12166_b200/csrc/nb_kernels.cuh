@@ -64,15 +64,9 @@ __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) {
     f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
 }
 
-// Packed operations that the compiler may neither reorder among themselves nor fold (see sym_step, sym_sweep).
-__device__ __forceinline__ f32x2 add2v(f32x2 a, f32x2 b) {
-    f32x2 d; asm volatile("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
-}
+// Packed operations that the compiler may neither reorder among themselves nor fold (see sym_step).
 __device__ __forceinline__ f32x2 fma2v(f32x2 a, f32x2 b, f32x2 c) {
     f32x2 d; asm volatile("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d;
-}
-__device__ __forceinline__ f32x2 mul2v(f32x2 a, f32x2 b) {
-    f32x2 d; asm volatile("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d;
 }
 
 // Radius of the star an element index belongs to (star 0 first, then star 1).
@@ -260,27 +254,31 @@ nb_gravity_kernel(const __grid_constant__ GravArgs a)
 // Eq. 4 is a force "between elements i and j": F_ij = -F_ji, so the geometric
 // factor c = 1/(r (r+eps)^2) and the difference d of a pair serve both a_i += G m_j c d and
 // a_j -= G m_i c d.  Elements are cut into super-tiles of S; one CTA owns one pair of
-// super-tiles (A <= B).  Each of its NT/32 warps keeps 64 H elements i of A in registers (2 H per
-// lane: H packed pairs) and walks the tiles of 64 elements j of B.  Inside a tile the warp
-// ROTATES: at step k lane l meets slots (l+k)&31 and 32+((l+k)&31) (conflict-free LDS.128),
-// accumulates a_i in its own registers and the pairs' reaction in six scalar registers that travel
-// with the slots (SHFL to lane l-1 after every step); after 32 steps the lane holds the finished
-// sums of slots l and 32+l over the warp's 64 H elements i and adds them to the CTA's shared-memory
-// array.  The warps of a CTA are skewed over different tiles and meet at a barrier after every
-// tile, so the shared-memory sums have a fixed order: results are bitwise reproducible.
-// Template parameters: S super-tile, H packed pairs of i per lane, NT threads, MINB CTAs/SM,
-//   JP    reaction summed in packed form (FMUL2/FFMA2 issued right behind the a_i FFMA2 of the same
-//         (c, d): both sources come from the operand reuse cache) and folded by two FADD, instead of
-//         one scalar FFMA per pair;
-//   MONT  reciprocal shared by the two j of a lane (as in the one-sided kernel) instead of one
-//         MUFU.RCP per pair;   UNR  unroll of the 32-step rotation.
-// Shipped: H = 2, JP, no MONT, UNR = 4 (DESIGN.md 5.1c lists what the others measured).  Per lane
-// and step (4 i x 2 j = 8 pairs = 16 interactions): 48 + 12 packed FP32 instructions, 12 FADD,
-// 16 MUFU, 6 SHFL, 2 LDS.128 -- 13.5 executed flop per interaction against 22 one-sided.
+// super-tiles (A <= B) and stages B in shared memory as PACKED PAIRS: pair p of tile t holds
+// elements 64 t + p and 64 t + 32 + p (float2 arrays X2, Y2, Z2, M2).  Each of its NT/32 warps
+// keeps 32 NI elements i of A in registers (NI per lane, as broadcast scalars) and walks the
+// tiles of B.  Inside a tile the warp ROTATES: at step k lane l meets pair (l+k)&31 (three
+// conflict-free LDS.64), so both accumulations are lane-aligned packed FFMA2 with the same
+// sources (c, d):  a_i += c d  into a per-i accumulator whose halves are the sums over the two
+// slot families (added once per round), and the reaction  a_j += c d  into one packed register
+// triple that TRAVELS WITH THE PAIR (SHFL to lane l-1 after every step).  The two FFMA2 are issued
+// back to back (asm volatile keeps the order): the second takes (c, d) from the operand reuse
+// cache and reads only its accumulator from the register file.  After 32 steps the lane holds the
+// finished reaction sums of pair l over the warp's 32 NI elements i and adds them to the CTA's
+// shared-memory array.  The warps of a CTA are skewed over different tiles and meet at a barrier
+// after every tile, so the shared-memory sums have a fixed order: bitwise reproducible.
+// Per lane and step at NI = 4 (4 i x 2 j = 8 pairs = 16 interactions): 60 packed FP32 instructions
+// (FADD2 x12, FFMA2 x12+4, FMUL2 x8, FFMA2 x12+12), 16 MUFU (one RSQ and one RCP per pair: a pair
+// evaluation already serves two interactions, so the shared reciprocal of the one-sided kernel
+// would cost more FMA-pipe cycles than the XU cycles it saves), 6 SHFL, 3 LDS.64 -- 13.5 executed
+// flop per interaction against 22 one-sided.  DESIGN.md 5.1c lists the variants measured on the way
+// (packed lanes along i with horizontal adds, Montgomery, NI, CTA shapes, unrolls).
 // Output: part[Y][e] = acceleration of element e due to the elements of super-tile Y (every
 // (Y, tile of e) combination is written by exactly one CTA; the diagonal CTAs (A == B) run the
 // one-sided loop).  Super-tiles of one mass take the mass out of the loop, as in
 // the one-sided kernel; other pairs of super-tiles multiply c by G m_j and G m_i per pair.
+// Template parameters: S super-tile, NI elements i per lane, NT threads, MINB CTAs/SM, UNR unroll
+// of the 32-step rotation.
 struct SymArgs {
     const float4* __restrict__ posm;   // [n] x,y,z,m
     float4* __restrict__ part;         // [T][n]
@@ -290,110 +288,55 @@ struct SymArgs {
 
 constexpr int kSymSmemPerElem = 28;    // dynamic shared memory of the symmetric kernel: (16 + 3*4) bytes x S
 
-template <int H, bool UNI, bool SYM, bool JP, bool MONT>
-__device__ __forceinline__ void sym_step(const float4 p0, const float4 p1,
-                                         const f32x2 (&nxi)[H], const f32x2 (&nyi)[H], const f32x2 (&nzi)[H],
-                                         const f32x2 (&gmi)[H], const f32x2 eps2,
-                                         f32x2 (&ax)[H], f32x2 (&ay)[H], f32x2 (&az)[H],
-                                         float (&ja)[3], float (&jb)[3])
+template <int NI, bool UNI, bool SYM>
+__device__ __forceinline__ void sym_step(const f32x2 X, const f32x2 Y, const f32x2 Z, const f32x2 M,
+                                          const float (&nxi)[NI], const float (&nyi)[NI], const float (&nzi)[NI],
+                                          const float (&gmi)[NI], const f32x2 eps2,
+                                          f32x2 (&ax)[NI], f32x2 (&ay)[NI], f32x2 (&az)[NI],
+                                          f32x2& jx, f32x2& jy, f32x2& jz)
 {
     const f32x2 tiny2 = pk2(kTinyR2, kTinyR2);
-    f32x2 ga[3], gb[3];                                                    // JP: packed reaction of this step
 #pragma unroll
-    for (int h = 0; h < H; ++h) {
-        const f32x2 dx0 = add2(pk2(p0.x, p0.x), nxi[h]), dy0 = add2(pk2(p0.y, p0.y), nyi[h]), dz0 = add2(pk2(p0.z, p0.z), nzi[h]);
-        const f32x2 dx1 = add2(pk2(p1.x, p1.x), nxi[h]), dy1 = add2(pk2(p1.y, p1.y), nyi[h]), dz1 = add2(pk2(p1.z, p1.z), nzi[h]);
-        f32x2 r20 = fma2(dx0, dx0, tiny2); r20 = fma2(dy0, dy0, r20); r20 = fma2(dz0, dz0, r20);
-        f32x2 r21 = fma2(dx1, dx1, tiny2); r21 = fma2(dy1, dy1, r21); r21 = fma2(dz1, dz1, r21);
-        float a0, b0, a1, b1;
-        unpk2(r20, a0, b0); unpk2(r21, a1, b1);
-        const f32x2 ri0 = pk2(rsqrt_approx(a0), rsqrt_approx(b0));         // 1/r
-        const f32x2 ri1 = pk2(rsqrt_approx(a1), rsqrt_approx(b1));
-        const f32x2 s0 = fma2(r20, ri0, eps2), s1 = fma2(r21, ri1, eps2);   // r + eps
-        const f32x2 t0 = mul2(s0, s0), t1 = mul2(s1, s1);                   // (r + eps)^2
-        f32x2 c0, c1;                                                      // 1/(r (r+eps)^2)   Eq. 4
-        if (MONT) {
-            const f32x2 P = mul2(t0, t1);
-            float pl, ph;
-            unpk2(P, pl, ph);
-            const f32x2 iP = pk2(rcp_approx(pl), rcp_approx(ph));          // one RCP per two pairs
-            const f32x2 k0 = mul2(t1, ri0), k1 = mul2(t0, ri1);
-            c0 = mul2(iP, k0); c1 = mul2(iP, k1);
+    for (int i = 0; i < NI; ++i) {
+        const f32x2 dx = add2(X, pk2(nxi[i], nxi[i])), dy = add2(Y, pk2(nyi[i], nyi[i])), dz = add2(Z, pk2(nzi[i], nzi[i]));
+        f32x2 r2 = fma2(dx, dx, tiny2); r2 = fma2(dy, dy, r2); r2 = fma2(dz, dz, r2);
+        float a0, b0;
+        unpk2(r2, a0, b0);
+        const f32x2 ri = pk2(rsqrt_approx(a0), rsqrt_approx(b0));          // 1/r
+        const f32x2 sm = fma2(r2, ri, eps2);                               // r + eps
+        const f32x2 t = mul2(sm, sm);                                      // (r + eps)^2
+        unpk2(t, a0, b0);
+        const f32x2 c = mul2(ri, pk2(rcp_approx(a0), rcp_approx(b0)));     // 1/(r (r+eps)^2)   Eq. 4
+        if (UNI) {
+            if (SYM) {
+                ax[i] = fma2v(c, dx, ax[i]); jx = fma2v(c, dx, jx);
+                ay[i] = fma2v(c, dy, ay[i]); jy = fma2v(c, dy, jy);
+                az[i] = fma2v(c, dz, az[i]); jz = fma2v(c, dz, jz);
+            } else {
+                ax[i] = fma2(c, dx, ax[i]); ay[i] = fma2(c, dy, ay[i]); az[i] = fma2(c, dz, az[i]);
+            }
         } else {
-            float l0, h0, l1, h1;
-            unpk2(t0, l0, h0); unpk2(t1, l1, h1);
-            c0 = mul2(ri0, pk2(rcp_approx(l0), rcp_approx(h0)));
-            c1 = mul2(ri1, pk2(rcp_approx(l1), rcp_approx(h1)));
-        }
-        f32x2 ci0 = c0, ci1 = c1, cj0 = c0, cj1 = c1;
-        if (!UNI) {
-            ci0 = mul2(c0, pk2(p0.w, p0.w)); ci1 = mul2(c1, pk2(p1.w, p1.w));   // G m_j for a_i
-            if (SYM) { cj0 = mul2(c0, gmi[h]); cj1 = mul2(c1, gmi[h]); }        // G m_i for a_j
-        }
-        if (SYM && JP && UNI) {
-            // a_i and the reaction use the same (c, d): issued back to back, the second instruction takes
-            // both from the operand reuse cache and reads only its accumulator from the register file
-            if (h == 0) {
-                ax[h] = fma2v(c0, dx0, ax[h]); ga[0] = mul2v(c0, dx0);
-                ay[h] = fma2v(c0, dy0, ay[h]); ga[1] = mul2v(c0, dy0);
-                az[h] = fma2v(c0, dz0, az[h]); ga[2] = mul2v(c0, dz0);
-                ax[h] = fma2v(c1, dx1, ax[h]); gb[0] = mul2v(c1, dx1);
-                ay[h] = fma2v(c1, dy1, ay[h]); gb[1] = mul2v(c1, dy1);
-                az[h] = fma2v(c1, dz1, az[h]); gb[2] = mul2v(c1, dz1);
-            } else {
-                ax[h] = fma2v(c0, dx0, ax[h]); ga[0] = fma2v(c0, dx0, ga[0]);
-                ay[h] = fma2v(c0, dy0, ay[h]); ga[1] = fma2v(c0, dy0, ga[1]);
-                az[h] = fma2v(c0, dz0, az[h]); ga[2] = fma2v(c0, dz0, ga[2]);
-                ax[h] = fma2v(c1, dx1, ax[h]); gb[0] = fma2v(c1, dx1, gb[0]);
-                ay[h] = fma2v(c1, dy1, ay[h]); gb[1] = fma2v(c1, dy1, gb[1]);
-                az[h] = fma2v(c1, dz1, az[h]); gb[2] = fma2v(c1, dz1, gb[2]);
+            const f32x2 ci = mul2(c, M);                                   // G m_j for a_i
+            ax[i] = fma2(ci, dx, ax[i]); ay[i] = fma2(ci, dy, ay[i]); az[i] = fma2(ci, dz, az[i]);
+            if (SYM) {
+                const f32x2 cj = mul2(c, pk2(gmi[i], gmi[i]));             // G m_i for a_j
+                jx = fma2(cj, dx, jx); jy = fma2(cj, dy, jy); jz = fma2(cj, dz, jz);
             }
-            continue;
-        }
-        ax[h] = fma2(ci0, dx0, ax[h]); ay[h] = fma2(ci0, dy0, ay[h]); az[h] = fma2(ci0, dz0, az[h]);
-        ax[h] = fma2(ci1, dx1, ax[h]); ay[h] = fma2(ci1, dy1, ay[h]); az[h] = fma2(ci1, dz1, az[h]);
-        if (SYM && !JP) {                                                  // reaction: a_j -= [G m_i] c d
-            float cl, ch, dl, dh;
-            unpk2(cj0, cl, ch);
-            unpk2(dx0, dl, dh); ja[0] = fmaf(cl, dl, ja[0]); ja[0] = fmaf(ch, dh, ja[0]);
-            unpk2(dy0, dl, dh); ja[1] = fmaf(cl, dl, ja[1]); ja[1] = fmaf(ch, dh, ja[1]);
-            unpk2(dz0, dl, dh); ja[2] = fmaf(cl, dl, ja[2]); ja[2] = fmaf(ch, dh, ja[2]);
-            unpk2(cj1, cl, ch);
-            unpk2(dx1, dl, dh); jb[0] = fmaf(cl, dl, jb[0]); jb[0] = fmaf(ch, dh, jb[0]);
-            unpk2(dy1, dl, dh); jb[1] = fmaf(cl, dl, jb[1]); jb[1] = fmaf(ch, dh, jb[1]);
-            unpk2(dz1, dl, dh); jb[2] = fmaf(cl, dl, jb[2]); jb[2] = fmaf(ch, dh, jb[2]);
-        }
-        if (SYM && JP) {
-            if (h == 0) {
-                ga[0] = mul2(cj0, dx0); ga[1] = mul2(cj0, dy0); ga[2] = mul2(cj0, dz0);
-                gb[0] = mul2(cj1, dx1); gb[1] = mul2(cj1, dy1); gb[2] = mul2(cj1, dz1);
-            } else {
-                ga[0] = fma2(cj0, dx0, ga[0]); ga[1] = fma2(cj0, dy0, ga[1]); ga[2] = fma2(cj0, dz0, ga[2]);
-                gb[0] = fma2(cj1, dx1, gb[0]); gb[1] = fma2(cj1, dy1, gb[1]); gb[2] = fma2(cj1, dz1, gb[2]);
-            }
-        }
-    }
-    if (SYM && JP) {
-#pragma unroll
-        for (int c = 0; c < 3; ++c) {
-            float l, h2;
-            unpk2(ga[c], l, h2); ja[c] = (ja[c] + l) + h2;
-            unpk2(gb[c], l, h2); jb[c] = (jb[c] + l) + h2;
         }
     }
 }
 
-// All tiles of super-tile B (in shared memory) against the warp's 64 H elements i, for every
-// round of elements i of super-tile A.
-template <int S, int H, int NT, bool JP, bool MONT, int UNR, bool UNI, bool SYM>
-__device__ __forceinline__ void sym_sweep(const SymArgs& a, const int A, const int B, const float4* __restrict__ jpos,
-                                          float* __restrict__ jax, float* __restrict__ jay, float* __restrict__ jaz,
-                                          const double scale_i)
+template <int S, int NI, int NT, int UNR, bool UNI, bool SYM>
+__device__ __forceinline__ void sym_sweep(const SymArgs& a, const int A, const int B,
+                                           const float2* __restrict__ X2, const float2* __restrict__ Y2,
+                                           const float2* __restrict__ Z2, const float2* __restrict__ M2,
+                                           float2* __restrict__ JX, float2* __restrict__ JY, float2* __restrict__ JZ,
+                                           const double scale_i)
 {
     constexpr int NW = NT / 32;
-    constexpr int NJT = S / 64;                      // tiles of 64 elements j
-    constexpr int SKEW = NJT / NW;                   // the warps of a CTA work on different tiles
-    constexpr int IPR = NW * 64 * H;                 // elements i per round
+    constexpr int NJT = S / 64;                      // tiles of 64 elements j = 32 packed pairs
+    constexpr int SKEW = NJT / NW;
+    constexpr int IPR = NW * 32 * NI;                // elements i per round
     static_assert(S % (64 * NW) == 0 && S % IPR == 0, "every warp needs its own tile at every step");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int src = (lane + 1) & 31;
@@ -402,81 +345,72 @@ __device__ __forceinline__ void sym_sweep(const SymArgs& a, const int A, const i
 
 #pragma unroll 1
     for (int r = 0; r < S / IPR; ++r) {
-        const int ibase = A * S + r * IPR + warp * (64 * H) + lane;
-        f32x2 nxi[H], nyi[H], nzi[H], gmi[H], rx[H], ry[H], rz[H];
+        const int ibase = A * S + r * IPR + warp * (32 * NI) + lane;
+        float nxi[NI], nyi[NI], nzi[NI], gmi[NI];
+        f32x2 ax[NI], ay[NI], az[NI];
 #pragma unroll
-        for (int h = 0; h < H; ++h) {
-            const int i0 = ibase + h * 64, i1 = i0 + 32;
-            float4 q0 = make_float4(kFarAway, kFarAway, kFarAway, 0.f), q1 = q0;
-            if (i0 < a.n) q0 = a.posm[i0];
-            if (i1 < a.n) q1 = a.posm[i1];
-            nxi[h] = pk2(-q0.x, -q1.x); nyi[h] = pk2(-q0.y, -q1.y); nzi[h] = pk2(-q0.z, -q1.z);
-            gmi[h] = pk2(a.G * q0.w, a.G * q1.w);
-            // define each packed pair by a packed instruction, so that it lives in one aligned
-            // register pair for the whole sweep (otherwise ptxas keeps the halves where the loads
-            // put them and re-packs them with two MOVs at every use)
-            const f32x2 zero2 = pk2(0.f, 0.f);
-            nxi[h] = add2v(nxi[h], zero2); nyi[h] = add2v(nyi[h], zero2); nzi[h] = add2v(nzi[h], zero2);
-            gmi[h] = add2v(gmi[h], zero2);
-            rx[h] = ry[h] = rz[h] = pk2(0.f, 0.f);
+        for (int i = 0; i < NI; ++i) {
+            const int e = ibase + i * 32;
+            float4 q = make_float4(kFarAway, kFarAway, kFarAway, 0.f);
+            if (e < a.n) q = a.posm[e];
+            nxi[i] = -q.x; nyi[i] = -q.y; nzi[i] = -q.z; gmi[i] = a.G * q.w;
+            ax[i] = ay[i] = az[i] = pk2(0.f, 0.f);
         }
-
 #pragma unroll 1
         for (int q = 0; q < NJT; ++q) {
             const int tile = (q + warp * SKEW) & (NJT - 1);
-            const float4* __restrict__ tp = jpos + tile * 64;
-            f32x2 ax[H], ay[H], az[H];
-#pragma unroll
-            for (int h = 0; h < H; ++h) ax[h] = ay[h] = az[h] = pk2(0.f, 0.f);
-            float ja[3] = {0.f, 0.f, 0.f}, jb[3] = {0.f, 0.f, 0.f};
+            const int tb = tile * 32;
+            f32x2 jx = pk2(0.f, 0.f), jy = jx, jz = jx;
 #pragma unroll UNR
             for (int k = 0; k < 32; ++k) {
-                const int slot = (lane + k) & 31;
-                sym_step<H, UNI, SYM, JP, MONT>(tp[slot], tp[32 + slot], nxi, nyi, nzi, gmi, eps2, ax, ay, az, ja, jb);
+                const int slot = tb + ((lane + k) & 31);
+                const f32x2 X = *reinterpret_cast<const f32x2*>(X2 + slot), Y = *reinterpret_cast<const f32x2*>(Y2 + slot),
+                            Z = *reinterpret_cast<const f32x2*>(Z2 + slot);
+                f32x2 M = 0;
+                if (!UNI) M = *reinterpret_cast<const f32x2*>(M2 + slot);
+                sym_step<NI, UNI, SYM>(X, Y, Z, M, nxi, nyi, nzi, gmi, eps2, ax, ay, az, jx, jy, jz);
                 if (SYM) {
-#pragma unroll
-                    for (int c = 0; c < 3; ++c) {
-                        ja[c] = __shfl_sync(0xffffffffu, ja[c], src);
-                        jb[c] = __shfl_sync(0xffffffffu, jb[c], src);
-                    }
+                    float l, h;
+                    unpk2(jx, l, h); jx = pk2(__shfl_sync(0xffffffffu, l, src), __shfl_sync(0xffffffffu, h, src));
+                    unpk2(jy, l, h); jy = pk2(__shfl_sync(0xffffffffu, l, src), __shfl_sync(0xffffffffu, h, src));
+                    unpk2(jz, l, h); jz = pk2(__shfl_sync(0xffffffffu, l, src), __shfl_sync(0xffffffffu, h, src));
                 }
             }
-#pragma unroll
-            for (int h = 0; h < H; ++h) {            // short fp32 chains: 64 terms per tile, then S/64 tile sums
-                rx[h] = add2(rx[h], ax[h]); ry[h] = add2(ry[h], ay[h]); rz[h] = add2(rz[h], az[h]);
-            }
-            if (SYM) {                               // after 32 rotations lane l holds slots l and 32+l
-                const int e = tile * 64 + lane;
-                jax[e] += ja[0]; jay[e] += ja[1]; jaz[e] += ja[2];
-                jax[e + 32] += jb[0]; jay[e + 32] += jb[1]; jaz[e + 32] += jb[2];
+            if (SYM) {                               // after 32 rotations lane l holds the pair of slots l, 32+l
+                float l, h;
+                float2 v;
+                v = JX[tb + lane]; unpk2(jx, l, h); v.x += l; v.y += h; JX[tb + lane] = v;
+                v = JY[tb + lane]; unpk2(jy, l, h); v.x += l; v.y += h; JY[tb + lane] = v;
+                v = JZ[tb + lane]; unpk2(jz, l, h); v.x += l; v.y += h; JZ[tb + lane] = v;
                 __syncthreads();                     // fixed order of the shared-memory sums
             }
         }
 #pragma unroll
-        for (int h = 0; h < H; ++h) {
-            const int i0 = ibase + h * 64, i1 = i0 + 32;
+        for (int i = 0; i < NI; ++i) {
+            const int e = ibase + i * 32;
             float xl, xh, yl, yh, zl, zh;
-            unpk2(rx[h], xl, xh); unpk2(ry[h], yl, yh); unpk2(rz[h], zl, zh);
-            if (i0 < a.n) out[i0] = make_float4((float)(scale_i * (double)xl), (float)(scale_i * (double)yl),
-                                                (float)(scale_i * (double)zl), 0.f);
-            if (i1 < a.n) out[i1] = make_float4((float)(scale_i * (double)xh), (float)(scale_i * (double)yh),
-                                                (float)(scale_i * (double)zh), 0.f);
+            unpk2(ax[i], xl, xh); unpk2(ay[i], yl, yh); unpk2(az[i], zl, zh);
+            if (e < a.n) out[e] = make_float4((float)(scale_i * ((double)xl + (double)xh)),
+                                              (float)(scale_i * ((double)yl + (double)yh)),
+                                              (float)(scale_i * ((double)zl + (double)zh)), 0.f);
         }
     }
 }
 
-template <int S, int H, int NT, int MINB, bool JP, bool MONT, int UNR = 2>
+template <int S, int NI, int NT, int MINB, int UNR>
 __global__ void __launch_bounds__(NT, MINB)
 nb_gravity_sym_kernel(const __grid_constant__ SymArgs a)
 {
-    extern __shared__ float4 sym_smem[];             // S float4 + 3 S float = 28 S bytes (dynamic: 56 KB at S = 2048)
-    float4* __restrict__ jpos = sym_smem;
-    float* __restrict__ jax = reinterpret_cast<float*>(sym_smem + S);
-    float* __restrict__ jay = jax + S;
-    float* __restrict__ jaz = jay + S;
+    extern __shared__ float4 sym_smem[];             // 7 arrays of S/2 float2 = 28 S bytes
+    float2* __restrict__ X2 = reinterpret_cast<float2*>(sym_smem);
+    float2* __restrict__ Y2 = X2 + S / 2;
+    float2* __restrict__ Z2 = Y2 + S / 2;
+    float2* __restrict__ M2 = Z2 + S / 2;
+    float2* __restrict__ JX = M2 + S / 2;
+    float2* __restrict__ JY = JX + S / 2;
+    float2* __restrict__ JZ = JY + S / 2;
     const int tid = threadIdx.x;
 
-    // block -> (A, B): the T(T-1)/2 off-diagonal pairs row by row, then the T diagonal ones
     int A, B;
     {
         const long long T = a.T, M = T * (T - 1) / 2, b = blockIdx.x;
@@ -492,36 +426,41 @@ nb_gravity_sym_kernel(const __grid_constant__ SymArgs a)
         }
     }
 
-    // stage super-tile B (G folded into m_j), clear its sums, and find out whether A and B
-    // are each made of one mass
+    // stage super-tile B as packed pairs: pair p of tile t holds elements 64 t + p and 64 t + 32 + p
     const float mB = a.posm[min(B * S, a.n - 1)].w, mA = a.posm[min(A * S, a.n - 1)].w;
     bool u = true;
-    for (int e = tid; e < S; e += NT) {
-        const int j = B * S + e, i = A * S + e;
-        float4 p = make_float4(kFarAway, kFarAway, kFarAway, 0.f);
-        if (j < a.n) { p = a.posm[j]; u = u && (p.w == mB); p.w *= a.G; } else u = false;
-        if (i < a.n) u = u && (a.posm[i].w == mA); else u = false;
-        jpos[e] = p;
-        jax[e] = 0.f; jay[e] = 0.f; jaz[e] = 0.f;
+    for (int p = tid; p < S / 2; p += NT) {
+        const int e0 = (p >> 5) * 64 + (p & 31), e1 = e0 + 32;
+        float4 q0 = make_float4(kFarAway, kFarAway, kFarAway, 0.f), q1 = q0;
+        if (B * S + e0 < a.n) { q0 = a.posm[B * S + e0]; u = u && (q0.w == mB); q0.w *= a.G; } else u = false;
+        if (B * S + e1 < a.n) { q1 = a.posm[B * S + e1]; u = u && (q1.w == mB); q1.w *= a.G; } else u = false;
+        if (A * S + e0 < a.n) u = u && (a.posm[A * S + e0].w == mA); else u = false;
+        if (A * S + e1 < a.n) u = u && (a.posm[A * S + e1].w == mA); else u = false;
+        X2[p] = make_float2(q0.x, q1.x); Y2[p] = make_float2(q0.y, q1.y); Z2[p] = make_float2(q0.z, q1.z);
+        M2[p] = make_float2(q0.w, q1.w);
+        JX[p] = JY[p] = JZ[p] = make_float2(0.f, 0.f);
     }
     const int uni = __syncthreads_and(u ? 1 : 0);
 
     if (A == B) {
-        if (uni) sym_sweep<S, H, NT, JP, MONT, UNR, true, false>(a, A, B, jpos, jax, jay, jaz, (double)(a.G * mB));
-        else     sym_sweep<S, H, NT, JP, MONT, UNR, false, false>(a, A, B, jpos, jax, jay, jaz, 1.0);
+        if (uni) sym_sweep<S, NI, NT, UNR, true, false>(a, A, B, X2, Y2, Z2, M2, JX, JY, JZ, (double)(a.G * mB));
+        else     sym_sweep<S, NI, NT, UNR, false, false>(a, A, B, X2, Y2, Z2, M2, JX, JY, JZ, 1.0);
         return;
     }
-    if (uni) sym_sweep<S, H, NT, JP, MONT, UNR, true, true>(a, A, B, jpos, jax, jay, jaz, (double)(a.G * mB));
-    else     sym_sweep<S, H, NT, JP, MONT, UNR, false, true>(a, A, B, jpos, jax, jay, jaz, 1.0);
+    if (uni) sym_sweep<S, NI, NT, UNR, true, true>(a, A, B, X2, Y2, Z2, M2, JX, JY, JZ, (double)(a.G * mB));
+    else     sym_sweep<S, NI, NT, UNR, false, true>(a, A, B, X2, Y2, Z2, M2, JX, JY, JZ, 1.0);
 
-    // reaction sums of super-tile B due to super-tile A (sign: a_j -= ...)
     const double scale_j = uni ? -(double)(a.G * mA) : -1.0;
     float4* __restrict__ outj = a.part + (size_t)A * a.n;
-    for (int e = tid; e < S; e += NT) {
-        const int j = B * S + e;
-        if (j < a.n)
-            outj[j] = make_float4((float)(scale_j * (double)jax[e]), (float)(scale_j * (double)jay[e]),
-                                  (float)(scale_j * (double)jaz[e]), 0.f);
+    for (int p = tid; p < S / 2; p += NT) {
+        const int e0 = (p >> 5) * 64 + (p & 31), e1 = e0 + 32;
+        const float2 x = JX[p], y = JY[p], z = JZ[p];
+        if (B * S + e0 < a.n)
+            outj[B * S + e0] = make_float4((float)(scale_j * (double)x.x), (float)(scale_j * (double)y.x),
+                                           (float)(scale_j * (double)z.x), 0.f);
+        if (B * S + e1 < a.n)
+            outj[B * S + e1] = make_float4((float)(scale_j * (double)x.y), (float)(scale_j * (double)y.y),
+                                           (float)(scale_j * (double)z.y), 0.f);
     }
 }
 
