@@ -218,3 +218,27 @@ def test_splat_argument_errors(nb):
     assert L.nb_splat(s.ctx, c3, 1.0, 0, 1, 8, 8, None) == nb.NB_EINVAL
     assert L.nb_splat(s.ctx, c3, 1.0, 0, 1, 8, 8, img.data_ptr()) == nb.NB_OK
     s.close()
+
+
+# ------------------------------------------------------------------ bench.py contract on the GPU
+def test_bench_line_has_the_contract_keys(nb):
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--steps", "3", "--warmup", "3",
+                          "--no-cpu-baseline"], capture_output=True, text=True, cwd=root, timeout=900)
+    assert out.returncode == 0, out.stderr[-2000:]
+    d = json.loads(out.stdout.strip().splitlines()[-1])
+    assert d["unit"] == "interactions/s" and d["n_gpus"] == 1 and d["steps"] == 3 and d["warmup"] == 3
+    assert d["higher_is_better"] is True and d["dtype"] == "f32" and d["data"] == "synthetic" and d["vs_baseline"] is None
+    assert d["config"]["workload"].startswith("config4") and d["config"]["n"] == 262144
+    assert d["value"] > 1e12 and abs(d["value"] - 262144.0 ** 2 / (d["ms_per_step"] * 1e-3)) < 1e-6 * d["value"]
+    r = d["roofline"]
+    assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and 0.3 < r["frac"] < 1.2 and r["frac_executed"] < r["frac"]
+    assert r["kernel"].startswith("nb_gravity_sym_kernel<1024") and 0.9 < r["kernel_share_of_step"] <= 1.0
+    assert abs(r["achieved"] / r["peak"] - r["frac"]) < 1e-9
+    e = d["e2e"]
+    assert e["h2d_bytes_per_step"] == e["d2h_bytes_per_step"] == 3 * 262144 * 16 and 0 < e["value"] < d["value"]
+    assert d["gpu_launches"] >= 3 * 3 and d["clocks"]["sm_mhz"] > 0
