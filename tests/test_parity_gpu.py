@@ -167,6 +167,31 @@ def test_symmetric_tile_bands(nb, n, name):
     _check_accel(nb, w, p, rows=_sample(w.n, 512, n))
 
 
+@pytest.mark.parametrize("seed", range(12))
+def test_symmetric_vs_one_sided_random_shapes(nb, seed):
+    """Random sizes (ragged against every tile size), star splits and mass patterns: the two gravity kernels
+    agree to fp32 rounding, the symmetric one obeys Newton's third law, and every third case also goes
+    against the full oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    n1, n2 = int(rng.integers(1, 4000)), int(rng.integers(1, 4000))
+    w = _ragged(n1, n2, seed=seed, eps=float(rng.choice([0.0, 0.003, 0.05])))
+    kind = seed % 3
+    if kind == 1:                                   # every element its own mass
+        w.posm[:, 3] *= rng.lognormal(0.0, 0.5, w.n).astype(np.float32)
+    elif kind == 2:                                 # a few heavy and a few massless elements inside uniform tiles
+        w.posm[rng.integers(0, w.n, 5), 3] *= np.float32(50.0)
+        w.posm[rng.integers(0, w.n, 5), 3] = 0.0
+    p = params_f32(dict(w.params, gamma=0.0))
+    a1, _ = _gpu_accel(nb, w, p, force_path=nb.NB_PATH_ONE_SIDED)
+    a2, _ = _gpu_accel(nb, w, p, force_path=nb.NB_PATH_SYMMETRIC)
+    scale = np.linalg.norm(a1, axis=1)
+    assert (np.linalg.norm(a1 - a2, axis=1) <= 1e-5 * scale + 1e-30).all()
+    m = w.posm[:, 3].astype(np.float64)
+    assert np.linalg.norm((m[:, None] * a2).sum(0)) <= 1e-5 * (m * np.linalg.norm(a2, axis=1)).sum()
+    if seed % 3 == 0:
+        _check_accel(nb, w, p, force_path=nb.NB_PATH_SYMMETRIC)
+
+
 def test_force_path_argument_errors(nb):
     w = make_config(1)
     s = _sim(nb, w)
