@@ -462,6 +462,36 @@ def test_long_run_invariants_config1(nb):
     assert e1["step"] == 300
 
 
+@pytest.mark.parametrize("idx", [3, 4])
+def test_full_length_runs_of_configs_3_and_4(nb, idx):
+    """A16: BASELINE's full runs (config 3: 1,000 steps with the donor's radius ramp; config 4: 100 steps) on the
+    symmetric kernel, judged by invariants: P and L conserved, no NaN, E not growing except through the work of
+    the ramp, the radii at their scheduled values, masses untouched, and (config 3) the filling donor starts to
+    lose elements across the L1 plane."""
+    w = make_config(idx)
+    p = params_f32(w.params)
+    nsteps = w.meta["nsteps"]
+    s = _sim(nb, w, p)
+    assert "sym" in nb.nb_force_kernel_name(s.ctx)
+    e0, t0 = s.energy(), s.transfer_diagnostics()
+    s.step(nsteps // 2); s.step(nsteps - nsteps // 2)
+    e1, t1 = s.energy(), s.transfer_diagnostics()
+    x = s.posm.cpu().numpy()
+    step, R = nb.nb_get_step(s.ctx)
+    s.close()
+    assert step == nsteps == e1["step"] and np.isfinite(x).all() and np.isfinite(e1["E"])
+    assert np.array_equal(x[:, 3], w.posm[:, 3])
+    assert np.array_equal(np.asarray(R, np.float32), np.asarray(p["R_end"], np.float32))
+    pscale = float((w.posm[:, 3] * np.linalg.norm(w.vel[:, :3], axis=1)).sum())
+    assert np.abs(np.array(e1["P"]) - np.array(e0["P"])).max() / pscale < 1e-5
+    assert abs(e1["L"][2] - e0["L"][2]) / abs(e0["L"][2]) < 1e-5
+    assert e1["Fnet"] < 1e-5 * 100
+    if idx == 4:                                    # no ramp: the inelastic contacts can only drain energy
+        assert e1["E"] < e0["E"] + 1e-4 * abs(e0["E"])
+    else:
+        assert t1["Mcross0"] >= t0["Mcross0"] and t1["M0"] == pytest.approx(t0["M0"], rel=1e-12)
+
+
 @pytest.mark.parametrize("path", [1, 2])
 def test_results_are_bitwise_reproducible(nb, path):
     """Both gravity kernels sum in a fixed order (no atomics): two runs give the same bits."""
