@@ -277,13 +277,17 @@ int launch_contact_on(nb_ctx* c, cudaStream_t st)
     if (c->n >= kSortMinN) {
         nb_bbox_kernel<<<kBoxBlocks, 256, 0, st>>>(c->posm, n, c->boxes());
         c->launches++;
-        nb_keys_kernel<<<(n + 255) / 256, 256, 0, st>>>(c->posm, n, c->boxes(), c->keys(), c->vals());
+        // cells per axis: ~16 per mean element spacing is plenty to order elements into compact groups, and
+        // every 8 key bits less is one pass less of the radix sort (n = 65,536: 30 bits, 4 passes instead of 6)
+        int bits = 4;
+        while ((1ll << (3 * (bits - 4))) < c->n && bits < kKeyBits) ++bits;
+        nb_keys_kernel<<<(n + 255) / 256, 256, 0, st>>>(c->posm, n, c->boxes(), c->keys(), c->vals(), bits);
         c->launches++;
         NB_CUDA(c, cudaGetLastError());
         cub::DoubleBuffer<unsigned long long> dk(c->keys(), c->keys() + c->n_max);
         cub::DoubleBuffer<uint32_t> dv(c->vals(), c->vals() + c->n_max);
         size_t tmp = c->lay.sorttmp_bytes;
-        NB_CUDA(c, cub::DeviceRadixSort::SortPairs(c->ws + c->lay.off_sorttmp, tmp, dk, dv, n, 0, 3 * kKeyBits, st));
+        NB_CUDA(c, cub::DeviceRadixSort::SortPairs(c->ws + c->lay.off_sorttmp, tmp, dk, dv, n, 0, 3 * bits, st));
         c->launches += 1;                              // counted as one (library) launch
         perm = dv.Current();
     }

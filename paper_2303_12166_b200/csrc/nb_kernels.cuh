@@ -529,14 +529,14 @@ __device__ __forceinline__ unsigned long long spread3(unsigned long long v) {
     return v;
 }
 
-constexpr int kKeyBits = 16;          // bits per axis; keys have 3*kKeyBits = 48 significant bits
+constexpr int kKeyBits = 16;          // most bits per axis; keys have at most 3*kKeyBits = 48 significant bits
 
-// Index of the cell (qx, qy, qz) along the 3-D Hilbert curve of order kKeyBits (Skilling's
+// Index of the cell (qx, qy, qz) along the 3-D Hilbert curve of order `bits` <= kKeyBits (Skilling's
 // axes-to-transpose transform, then bit interleave).  Unlike the Z-order curve it has no
 // jumps, so 32 consecutive elements always form a compact group.
-__device__ __forceinline__ unsigned long long hilbert_key(uint32_t qx, uint32_t qy, uint32_t qz) {
+__device__ __forceinline__ unsigned long long hilbert_key(uint32_t qx, uint32_t qy, uint32_t qz, int bits) {
     uint32_t X[3] = {qx, qy, qz};
-    for (uint32_t Q = 1u << (kKeyBits - 1); Q > 1; Q >>= 1) {
+    for (uint32_t Q = 1u << (bits - 1); Q > 1; Q >>= 1) {
         const uint32_t P = Q - 1;
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
@@ -546,7 +546,7 @@ __device__ __forceinline__ unsigned long long hilbert_key(uint32_t qx, uint32_t 
     }
     X[1] ^= X[0]; X[2] ^= X[1];
     uint32_t t = 0;
-    for (uint32_t Q = 1u << (kKeyBits - 1); Q > 1; Q >>= 1)
+    for (uint32_t Q = 1u << (bits - 1); Q > 1; Q >>= 1)
         if (X[2] & Q) t ^= Q - 1;
     X[0] ^= t; X[1] ^= t; X[2] ^= t;
     return (spread3(X[0]) << 2) | (spread3(X[1]) << 1) | spread3(X[2]);
@@ -554,10 +554,10 @@ __device__ __forceinline__ unsigned long long hilbert_key(uint32_t qx, uint32_t 
 
 __global__ void __launch_bounds__(256)
 nb_keys_kernel(const float4* __restrict__ posm, int n, const float4* __restrict__ boxes,
-               unsigned long long* __restrict__ keys, uint32_t* __restrict__ vals)
+               unsigned long long* __restrict__ keys, uint32_t* __restrict__ vals, int bits)
 {
     __shared__ float sh[4];
-    constexpr float kCells = (float)((1 << kKeyBits) - 1);
+    const float kCells = (float)((1 << bits) - 1);
     if (threadIdx.x < 32) {                       // reduce the kBoxBlocks partial boxes (cubic cells)
         float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
         for (int b = threadIdx.x; b < kBoxBlocks; b += 32) {
@@ -583,7 +583,7 @@ nb_keys_kernel(const float4* __restrict__ posm, int n, const float4* __restrict_
     const uint32_t qx = (uint32_t)fminf(fmaxf((p.x - sh[0]) * sc, 0.f), kCells);
     const uint32_t qy = (uint32_t)fminf(fmaxf((p.y - sh[1]) * sc, 0.f), kCells);
     const uint32_t qz = (uint32_t)fminf(fmaxf((p.z - sh[2]) * sc, 0.f), kCells);
-    keys[i] = hilbert_key(qx, qy, qz);
+    keys[i] = hilbert_key(qx, qy, qz, bits);
     vals[i] = (uint32_t)i;
 }
 
