@@ -78,8 +78,9 @@ typedef struct {
 int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream);
 
 /* Bytes of device workspace nb_set_state() needs for a context of n_max elements
- * (cached acceleration, partial sums of the gravity kernel -- up to 385 slabs of n float4 for the
- * symmetric kernel, i.e. ~6.2 KB per element --, device-side step/radius state,
+ * (cached acceleration, partial sums of the gravity kernel -- up to 513 slabs of n float4 for the
+ * symmetric kernel: 2-8 KB per element, 1.0 GiB at n_max = 262144, 4.6 GiB at 1048576 --, device-side
+ * step/radius state,
  * reduction scratch, and the contact pass's Hilbert keys, sort scratch, ordered copy and
  * group boxes).  0 if n_max is out of range. */
 size_t nb_workspace_bytes(int64_t n_max);
