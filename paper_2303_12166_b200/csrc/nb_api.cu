@@ -230,11 +230,11 @@ bool params_ok(const nb_params* p)
 }
 
 // The instantiations of the symmetric kernel: <S, elements i per lane, threads, CTAs/SM, unroll>.
-#define NB_SYM_256  nb_gravity_sym_kernel<256, 4, 64, 8, 4>
-#define NB_SYM_512  nb_gravity_sym_kernel<512, 4, 128, 4, 4>
-#define NB_SYM_1024 nb_gravity_sym_kernel<1024, 4, 256, 2, 4>
-#define NB_SYM_2048 nb_gravity_sym_kernel<2048, 4, 256, 2, 4>
-#define NB_SYM_4096 nb_gravity_sym_kernel<4096, 4, 256, 2, 4>
+#define NB_SYM_256  nb_gravity_sym_kernel<256, 4, 64, 8, 8>
+#define NB_SYM_512  nb_gravity_sym_kernel<512, 4, 128, 4, 8>
+#define NB_SYM_1024 nb_gravity_sym_kernel<1024, 4, 256, 2, 8>
+#define NB_SYM_2048 nb_gravity_sym_kernel<2048, 4, 256, 2, 8>
+#define NB_SYM_4096 nb_gravity_sym_kernel<4096, 4, 256, 2, 8>
 
 // Row a2: partial gravitational accelerations -> part[0..ngrav-1][n]
 //   symmetric kernel: one CTA per pair of super-tiles, part[Y][e] = a_e due to super-tile Y
@@ -731,11 +731,11 @@ int nb_set_force_path(nb_ctx* c, int path)
 const char* nb_force_kernel_name(nb_ctx* c)
 {
     if (!c || !c->have_state) return "";
-    if (c->plan.sym_S == 256) return "nb_gravity_sym_kernel<256,4,64,8,4>";
-    if (c->plan.sym_S == 512) return "nb_gravity_sym_kernel<512,4,128,4,4>";
-    if (c->plan.sym_S == 1024) return "nb_gravity_sym_kernel<1024,4,256,2,4>";
-    if (c->plan.sym_S == 2048) return "nb_gravity_sym_kernel<2048,4,256,2,4>";
-    if (c->plan.sym_S) return "nb_gravity_sym_kernel<4096,4,256,2,4>";
+    if (c->plan.sym_S == 256) return "nb_gravity_sym_kernel<256,4,64,8,8>";
+    if (c->plan.sym_S == 512) return "nb_gravity_sym_kernel<512,4,128,4,8>";
+    if (c->plan.sym_S == 1024) return "nb_gravity_sym_kernel<1024,4,256,2,8>";
+    if (c->plan.sym_S == 2048) return "nb_gravity_sym_kernel<2048,4,256,2,8>";
+    if (c->plan.sym_S) return "nb_gravity_sym_kernel<4096,4,256,2,8>";
     return c->plan.TJ == 256 ? "nb_gravity_kernel<2,256>" : "nb_gravity_kernel<2,128>";
 }
 

@@ -278,7 +278,8 @@ nb_gravity_kernel(const __grid_constant__ GravArgs a)
 // one-sided loop).  Super-tiles of one mass take the mass out of the loop, as in
 // the one-sided kernel; other pairs of super-tiles multiply c by G m_j and G m_i per pair.
 // Template parameters: S super-tile, NI elements i per lane, NT threads, MINB CTAs/SM, UNR unroll
-// of the 32-step rotation.
+// of the 32-step rotation (shipped: 8).  A step is written phase by phase over the NI elements i
+// (d and r^2 of all, then all MUFU.RSQ, ...), which keeps the MUFU of all of them in flight together.
 struct SymArgs {
     const float4* __restrict__ posm;   // [n] x,y,z,m
     float4* __restrict__ part;         // [T][n]
@@ -290,37 +291,52 @@ constexpr int kSymSmemPerElem = 28;    // dynamic shared memory of the symmetric
 
 template <int NI, bool UNI, bool SYM>
 __device__ __forceinline__ void sym_step(const f32x2 X, const f32x2 Y, const f32x2 Z, const f32x2 M,
-                                          const float (&nxi)[NI], const float (&nyi)[NI], const float (&nzi)[NI],
-                                          const float (&gmi)[NI], const f32x2 eps2,
-                                          f32x2 (&ax)[NI], f32x2 (&ay)[NI], f32x2 (&az)[NI],
-                                          f32x2& jx, f32x2& jy, f32x2& jz)
+                                         const float (&nxi)[NI], const float (&nyi)[NI], const float (&nzi)[NI],
+                                         const float (&gmi)[NI], const f32x2 eps2,
+                                         f32x2 (&ax)[NI], f32x2 (&ay)[NI], f32x2 (&az)[NI],
+                                         f32x2& jx, f32x2& jy, f32x2& jz)
 {
     const f32x2 tiny2 = pk2(kTinyR2, kTinyR2);
+    f32x2 dx[NI], dy[NI], dz[NI], r2[NI], ri[NI], t[NI], c[NI];
+    // phase by phase over the NI elements i, so that the MUFU of all of them are in flight together
 #pragma unroll
     for (int i = 0; i < NI; ++i) {
-        const f32x2 dx = add2(X, pk2(nxi[i], nxi[i])), dy = add2(Y, pk2(nyi[i], nyi[i])), dz = add2(Z, pk2(nzi[i], nzi[i]));
-        f32x2 r2 = fma2(dx, dx, tiny2); r2 = fma2(dy, dy, r2); r2 = fma2(dz, dz, r2);
+        dx[i] = add2(X, pk2(nxi[i], nxi[i])); dy[i] = add2(Y, pk2(nyi[i], nyi[i])); dz[i] = add2(Z, pk2(nzi[i], nzi[i]));
+        r2[i] = fma2(dx[i], dx[i], tiny2); r2[i] = fma2(dy[i], dy[i], r2[i]); r2[i] = fma2(dz[i], dz[i], r2[i]);
+    }
+#pragma unroll
+    for (int i = 0; i < NI; ++i) {
         float a0, b0;
-        unpk2(r2, a0, b0);
-        const f32x2 ri = pk2(rsqrt_approx(a0), rsqrt_approx(b0));          // 1/r
-        const f32x2 sm = fma2(r2, ri, eps2);                               // r + eps
-        const f32x2 t = mul2(sm, sm);                                      // (r + eps)^2
-        unpk2(t, a0, b0);
-        const f32x2 c = mul2(ri, pk2(rcp_approx(a0), rcp_approx(b0)));     // 1/(r (r+eps)^2)   Eq. 4
+        unpk2(r2[i], a0, b0);
+        ri[i] = pk2(rsqrt_approx(a0), rsqrt_approx(b0));                   // 1/r
+    }
+#pragma unroll
+    for (int i = 0; i < NI; ++i) {
+        const f32x2 sm = fma2(r2[i], ri[i], eps2);                         // r + eps
+        t[i] = mul2(sm, sm);                                               // (r + eps)^2
+    }
+#pragma unroll
+    for (int i = 0; i < NI; ++i) {
+        float a0, b0;
+        unpk2(t[i], a0, b0);
+        c[i] = mul2(ri[i], pk2(rcp_approx(a0), rcp_approx(b0)));           // 1/(r (r+eps)^2)   Eq. 4
+    }
+#pragma unroll
+    for (int i = 0; i < NI; ++i) {
         if (UNI) {
             if (SYM) {
-                ax[i] = fma2v(c, dx, ax[i]); jx = fma2v(c, dx, jx);
-                ay[i] = fma2v(c, dy, ay[i]); jy = fma2v(c, dy, jy);
-                az[i] = fma2v(c, dz, az[i]); jz = fma2v(c, dz, jz);
+                ax[i] = fma2v(c[i], dx[i], ax[i]); jx = fma2v(c[i], dx[i], jx);
+                ay[i] = fma2v(c[i], dy[i], ay[i]); jy = fma2v(c[i], dy[i], jy);
+                az[i] = fma2v(c[i], dz[i], az[i]); jz = fma2v(c[i], dz[i], jz);
             } else {
-                ax[i] = fma2(c, dx, ax[i]); ay[i] = fma2(c, dy, ay[i]); az[i] = fma2(c, dz, az[i]);
+                ax[i] = fma2(c[i], dx[i], ax[i]); ay[i] = fma2(c[i], dy[i], ay[i]); az[i] = fma2(c[i], dz[i], az[i]);
             }
         } else {
-            const f32x2 ci = mul2(c, M);                                   // G m_j for a_i
-            ax[i] = fma2(ci, dx, ax[i]); ay[i] = fma2(ci, dy, ay[i]); az[i] = fma2(ci, dz, az[i]);
+            const f32x2 ci = mul2(c[i], M);                                // G m_j for a_i
+            ax[i] = fma2(ci, dx[i], ax[i]); ay[i] = fma2(ci, dy[i], ay[i]); az[i] = fma2(ci, dz[i], az[i]);
             if (SYM) {
-                const f32x2 cj = mul2(c, pk2(gmi[i], gmi[i]));             // G m_i for a_j
-                jx = fma2(cj, dx, jx); jy = fma2(cj, dy, jy); jz = fma2(cj, dz, jz);
+                const f32x2 cj = mul2(c[i], pk2(gmi[i], gmi[i]));          // G m_i for a_j
+                jx = fma2(cj, dx[i], jx); jy = fma2(cj, dy[i], jy); jz = fma2(cj, dz[i], jz);
             }
         }
     }
