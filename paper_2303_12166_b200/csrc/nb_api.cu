@@ -304,7 +304,7 @@ int launch_contact_on(nb_ctx* c, cudaStream_t st)
     ca.v_dead = c->prm.v_dead; ca.lens_mode = c->prm.lens_mode;
     const int nchunks = c->ncontact();
     const long long warps = (long long)ngroups * nchunks;
-    ca.nchunks = nchunks; ca.spc = (nsuper + nchunks - 1) / nchunks;
+    ca.nchunks = nchunks;
     if (perm) {
         nb_contact_kernel<<<(int)((warps * 32 + kThreads - 1) / kThreads), kThreads, 0, st>>>(ca);
     } else {

@@ -653,9 +653,9 @@ struct ContactArgs {
     const float4* __restrict__ sbox;   // [2*nsuper]
     float4* __restrict__ out;          // [nchunks][n] contact acceleration, ORIGINAL index order
     int n, ngroups, nsuper;
-    int nchunks, spc;                  // nb_contact_kernel: the candidate groups of a group of elements i are dealt
+    int nchunks;                       // nb_contact_kernel: the candidate groups of a group of elements i are dealt
                                        // round-robin to nchunks warps (neighbours are adjacent on the Hilbert curve, so
-                                       // a split by ranges would leave all the work with one warp); spc unused
+                                       // a split by ranges would leave all the work with one warp)
     float gamma, gamma_beta;           // Eq. 5 / Eq. 6 strengths
     float v_dead;
     int lens_mode;
