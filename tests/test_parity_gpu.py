@@ -619,3 +619,29 @@ def test_steps_can_be_captured_in_a_cuda_graph(nb, idx, scale):
     assert nb.nb_get_step(s.ctx) == nb.nb_get_step(ref.ctx)
     assert nb.nb_get_step(s.ctx)[0] == 7
     s.close(); ref.close()
+
+
+def test_rebinding_states_of_different_size_in_one_context(nb):
+    """One context (n_max = 70,000) bound in turn to states of 30,000 (symmetric kernel, S = 256), 3,000 (one-sided
+    kernel) and 65,536 elements (S = 512): each gives the bits of a fresh context of its own size."""
+    import torch
+    ws = [_ragged(20000, 10000, seed=31), _ragged(1800, 1200, seed=32), make_config(3)]
+    n_max = 70000
+    p0 = params_f32(ws[0].params)
+    dev = torch.device("cuda:0")
+    work = torch.empty(nb.nb_workspace_bytes(n_max), dtype=torch.uint8, device=dev)
+    ctx = nb.nb_create(n_max, p0, torch.cuda.current_stream(dev).cuda_stream)
+    for w in ws:
+        p = params_f32(dict(w.params, **{k: p0[k] for k in ("G", "eps", "dt", "q", "gamma", "beta", "v_dead", "lens_mode",
+                                                            "R_start", "R_end", "n_ramp")}))
+        posm = torch.as_tensor(w.posm).to(dev); vel = torch.as_tensor(w.vel).to(dev); star = torch.as_tensor(w.star).to(dev)
+        nb.nb_set_state(ctx, w.n, posm, vel, star, work)
+        nb.nb_step(ctx, 2)
+        ref = nb.Simulation(w.posm, w.vel, w.star, p)
+        ref.step(2); ref.synchronize()
+        torch.cuda.synchronize()
+        assert nb.nb_force_kernel_name(ctx) == nb.nb_force_kernel_name(ref.ctx)
+        assert torch.equal(posm, ref.posm) and torch.equal(vel, ref.vel)
+        assert nb.nb_get_step(ctx)[0] == 2
+        ref.close()
+    nb.nb_destroy(ctx)
