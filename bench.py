@@ -267,6 +267,8 @@ def run_own(args):
                 "frac_executed": achieved / peak_tflops * executed / FLOP_PER_INTERACTION,
                 "pair_evaluations": "each unordered pair once (Newton's third law)" if symmetric
                                     else "every ordered pair",
+                "note": "achieved/frac use the ALGORITHMIC 21 flop per ordered interaction (SURVEY 8d); the symmetric "
+                        "kernel evaluates half of them, so frac can reach 1 -- frac_executed is what the ALUs did",
                 "kernel_share_of_step": k_ms / step_ms,
                 "contact_pass_ms": c_ms, "contact_pass_share_of_step": c_ms / step_ms,
                 "interactions_per_s": float(n) * n / (k_ms * 1e-3),
