@@ -748,15 +748,31 @@ __device__ __forceinline__ void contact_candidates(const ContactArgs& a, const i
         if (!__any_sync(0xffffffffu, valid && point_gap2(pi, lo, hi) <= Db * Db * kSlack)) continue;
         const int j0 = jg * kGroup;
         const int jn = min(kGroup, a.n - j0);
+        // stage the group as four arrays of 32 floats (x, y, z, R; the ragged end far away), so that one
+        // broadcast LDS.64 gives a packed pair of elements j and the pre-test runs on FADD2/FFMA2/FMUL2:
+        // the same operations in the same order per element as the scalar form, two elements at a time
+        float* __restrict__ sx = reinterpret_cast<float*>(stage);
         __syncwarp();
-        if (lane < jn) stage[lane] = a.ps[j0 + lane];
+        {
+            float4 p = make_float4(kFarAway, kFarAway, kFarAway, 0.f);
+            if (lane < jn) p = a.ps[j0 + lane];
+            sx[lane] = p.x; sx[32 + lane] = p.y; sx[64 + lane] = p.z; sx[96 + lane] = p.w;
+        }
         __syncwarp();
-        for (int t = 0; t < jn; ++t) {
-            const float4 pj = stage[t];
-            const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
-            const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            const float D = pi.w + pj.w;
-            if (r2 <= D * D * kSlack && valid) { hq[nh * 32 + lane] = (uint32_t)(j0 + t); ++nh; }
+        const f32x2 nx = pk2(-pi.x, -pi.x), ny = pk2(-pi.y, -pi.y), nz = pk2(-pi.z, -pi.z), Ri = pk2(pi.w, pi.w);
+        const f32x2 slack2 = pk2(kSlack, kSlack);
+#pragma unroll 4
+        for (int t = 0; t < kGroup; t += 2) {
+            const f32x2 dx = add2(*reinterpret_cast<const f32x2*>(sx + t), nx);
+            const f32x2 dy = add2(*reinterpret_cast<const f32x2*>(sx + 32 + t), ny);
+            const f32x2 dz = add2(*reinterpret_cast<const f32x2*>(sx + 64 + t), nz);
+            const f32x2 r2 = fma2(dz, dz, fma2(dy, dy, mul2(dx, dx)));
+            const f32x2 D = add2(Ri, *reinterpret_cast<const f32x2*>(sx + 96 + t));
+            const f32x2 thr = mul2(mul2(D, D), slack2);
+            float r0, r1, t0, t1;
+            unpk2(r2, r0, r1); unpk2(thr, t0, t1);
+            if (r0 <= t0 && valid) { hq[nh * 32 + lane] = (uint32_t)(j0 + t); ++nh; }
+            if (r1 <= t1 && valid) { hq[nh * 32 + lane] = (uint32_t)(j0 + t + 1); ++nh; }
         }
         if (__any_sync(0xffffffffu, nh >= kHitFlush)) contact_drain(a, hq, nh, pi, vi, lane, ax, ay, az);
     }
