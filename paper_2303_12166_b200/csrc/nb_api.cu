@@ -661,8 +661,8 @@ int nb_energy(nb_ctx* c, double* out)
     for (int b = 0; b < pot_blocks; ++b) { ug2 += hp[2 * b]; ur2 += hp[2 * b + 1]; }
     delete[] h;
     out[0] = m[0];
-    out[1] = -0.5 * ug2;
-    out[2] = 0.5 * ur2;
+    out[1] = -ug2;
+    out[2] = ur2;
     out[3] = out[0] + out[1] + out[2];
     for (int k = 0; k < 6; ++k) out[4 + k] = m[1 + k];
     out[10] = std::sqrt(m[7] * m[7] + m[8] * m[8] + m[9] * m[9]);

@@ -993,8 +993,9 @@ nb_moments_kernel(const float4* __restrict__ posm, const float4* __restrict__ ve
     }
 }
 
-// Potential energies: per block, sum_i m_i * sum_{j != i} G m_j/(r+eps)  and
-// sum_i sum_{j != i, contact} U_rep(r; R_ij)   (each unordered pair counted twice).
+// Potential energies: per block, sum_i m_i * sum_{j > i} G m_j/(r+eps)  and
+// sum_i sum_{j > i, contact} U_rep(r; R_ij)   (each unordered pair counted once: thread i walks only
+// the tiles from its own on; the blocks are launched in index order, longest first).
 struct PotArgs {
     const float4* __restrict__ posm;
     const DevState* __restrict__ dev;
@@ -1019,7 +1020,7 @@ nb_potential_kernel(const __grid_constant__ PotArgs a)
     const float kPi = 3.14159265358979f;
     double phi = 0.0, urep = 0.0;
     const int njt = (a.n + TJ - 1) / TJ;
-    for (int t = 0; t < njt; ++t) {
+    for (int t = (blockIdx.x * kThreads) / TJ; t < njt; ++t) {    // only the tiles that hold some j > i
         __syncthreads();
         for (int l = tid; l < TJ; l += kThreads) {
             const int j = t * TJ + l;
@@ -1034,9 +1035,9 @@ nb_potential_kernel(const __grid_constant__ PotArgs a)
             const float dx = pj.x - pi.x, dy = pj.y - pi.y, dz = pj.z - pi.z;
             const float r2 = fmaf(dz, dz, fmaf(dy, dy, fmaf(dx, dx, kTinyR2)));
             const float r = r2 * rsqrt_approx(r2);
-            const float w = (j == i) ? 0.f : pj.w;
+            const float w = (j > i) ? pj.w : 0.f;                    // every unordered pair once
             ph = fmaf(w, rcp_approx(r + a.eps), ph);
-            if (a.gamma > 0.f && r2 < Dmax * Dmax && j != i && j < a.n) {
+            if (a.gamma > 0.f && r2 < Dmax * Dmax && j > i && j < a.n) {
                 const float D = Ri + star_radius(j, a.n1, R0, R1);
                 const float rr = sqrtf(r2);
                 if (rr < D) {
