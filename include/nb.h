@@ -142,6 +142,13 @@ int nb_splat(nb_ctx* ctx, const float* centre, float half_width, int axis_u, int
  * Synchronises the stream. */
 int nb_get_step(nb_ctx* ctx, int64_t* step, float* R);
 
+/* Restore the step count n of a checkpointed run (the element radius is a function of
+ * how far the run has come): sets n = step and R_s(n) by the expanding-star rule, exactly as nsteps
+ * calls of nb_step() from 0 would have left them.  The full state of a run is (x, v, a(x_n), n):
+ * nb_upload_state() restores the arrays, this call the count.  The cached acceleration is kept (it
+ * belongs to the uploaded state).  step >= 0.  Asynchronous on the stream. */
+int nb_set_step(nb_ctx* ctx, int64_t step);
+
 /* Host-buffer entry points for end-to-end use and checkpoint/restart: copy HOST
  * float[n][4] arrays into / out of the bound device buffers on the ctx stream.
  * The full state of a run is (x, v, a(x_n), n): host_acc carries the cached

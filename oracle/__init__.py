@@ -41,6 +41,8 @@ def load():
         lib.orc_accel.restype = None
         lib.orc_accel.argtypes = [C.c_int64, dp, dp, dp, ip, dp, C.POINTER(_Params),
                                   C.c_int64, lp, dp, dp, dp]
+        lib.orc_contact_list.restype = None
+        lib.orc_contact_list.argtypes = [C.c_int64, dp, dp, ip, dp, C.c_int64, lp, C.c_int64, lp, lp, dp, dp]
         lib.orc_radii.restype = None
         lib.orc_radii.argtypes = [C.c_int64, dp, dp, C.c_int64, dp]
         lib.orc_step.restype = None
@@ -117,6 +119,29 @@ def accel(pos, vel, mass, star, R, params, rows=None, want_diag: bool = False):
                      _dp(Rr), C.byref(prm), nr, rp, _dp(a),
                      _dp(kap) if want_diag else None, _dp(dl) if want_diag else None)
     return (a, kap, dl) if want_diag else a
+
+
+def contact_list(pos, vel, star, R, rows=None, cap: int = 64):
+    """Contact pairs (r < R_i + R_j, A2/A3) of the elements in rows (all if None).
+    Returns count [nrows] (all pairs of the row), and j [nrows,cap] (-1 beyond count), r, rdot
+    [nrows,cap] (NaN beyond count) holding the first `cap` pairs of every row in j order."""
+    x, v = _f64(pos, 3), _f64(vel, 3)
+    st = np.ascontiguousarray(star, dtype=np.int32)
+    Rr = _f64(R)
+    n = x.shape[0]
+    lp = C.POINTER(C.c_int64)
+    if rows is None:
+        nr, rp = n, None
+    else:
+        rows = np.ascontiguousarray(rows, dtype=np.int64)
+        nr, rp = rows.shape[0], rows.ctypes.data_as(lp)
+    count = np.zeros(nr, np.int64)
+    jj = np.full((nr, cap), -1, np.int64)
+    rr = np.full((nr, cap), np.nan)
+    rd = np.full((nr, cap), np.nan)
+    load().orc_contact_list(n, _dp(x), _dp(v), st.ctypes.data_as(C.POINTER(C.c_int32)), _dp(Rr), nr, rp,
+                            int(cap), count.ctypes.data_as(lp), jj.ctypes.data_as(lp), _dp(rr), _dp(rd))
+    return count, jj, rr, rd
 
 
 class Sim:
@@ -255,3 +280,32 @@ def splat(pos, star, centre, half_width: float, axis_u: int, axis_v: int, W: int
     img = np.zeros((2, H, W), dtype=np.uint32)
     np.add.at(img, (st[ok], pv[ok].astype(np.int64), pu[ok].astype(np.int64)), 1)
     return img
+
+
+def splat_exact(pos, star, centre, half_width: float, axis_u: int, axis_v: int, W: int, H: int):
+    """f4 by its DEFINITION (reading A19), in float64 on the float32 inputs: element i lands in pixel
+    (floor(t_u), floor(t_v)), t_u = (x_u - c_u) W/(2 half_width) + W/2, t_v = (x_v - c_v) W/(2 half_width) + H/2
+    (square pixels), counted in image[star][py][px] if inside the window.
+
+    A float32 evaluation of t (four roundings: the difference, the scale W/(2 hw), the product, the sum) is off
+    by at most 2^-24 (3 |t - W/2| + |t|) <= 3 W 2^-24 pixels inside the window, so an element whose t lies
+    within that band of an integer may legitimately land in the neighbouring pixel (or across the window's
+    edge).  Returns (image uint32 [2,H,W], ambiguous uint32 [2,H+2,W+2]): ambiguous counts those elements in
+    their exact pixel, on a grid padded by one pixel on every side (index +1) so that elements just outside
+    the window are kept too."""
+    p = np.asarray(pos)[:, :3].astype(np.float32).astype(np.float64)
+    st = np.asarray(star).astype(np.int64)
+    c = np.asarray(centre, dtype=np.float32).astype(np.float64)
+    s = float(W) / (2.0 * float(np.float32(half_width)))
+    tu = (p[:, axis_u] - c[axis_u]) * s + 0.5 * W
+    tv = (p[:, axis_v] - c[axis_v]) * s + 0.5 * H
+    pu, pv = np.floor(tu), np.floor(tv)
+    ok = (pu >= 0) & (pu < W) & (pv >= 0) & (pv < H)
+    img = np.zeros((2, H, W), dtype=np.uint32)
+    np.add.at(img, (st[ok], pv[ok].astype(np.int64), pu[ok].astype(np.int64)), 1)
+    band_u, band_v = 3.0 * W * 2.0 ** -24, 3.0 * max(W, H) * 2.0 ** -24
+    near = (np.abs(tu - np.rint(tu)) <= band_u) | (np.abs(tv - np.rint(tv)) <= band_v)
+    keep = near & (pu >= -1) & (pu <= W) & (pv >= -1) & (pv <= H)
+    amb = np.zeros((2, H + 2, W + 2), dtype=np.uint32)
+    np.add.at(amb, (st[keep], pv[keep].astype(np.int64) + 1, pu[keep].astype(np.int64) + 1), 1)
+    return img, amb

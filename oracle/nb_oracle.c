@@ -121,6 +121,44 @@ void orc_accel(int64_t n, const double *x, const double *v, const double *m,
     }
 }
 
+/*
+ * The contact pairs of the elements listed in rows[0..nrows) (rows == NULL: all n): every j != i
+ * with 0 < r < R_i + R_j ("in contact"; A2, A3), in j order.  count[k] receives the
+ * number of such pairs of row k; the first min(count[k], cap) of them are written to
+ * jj / rr / rd [k*cap + ...] as (j, r, rdot = d.(v_j - v_i)/r) -- the quantity whose sign selects
+ * Eq. 5 or Eq. 6 (A5).  No force arithmetic here: the tests use the list to derive,
+ * from the distribution of rdot, how many pairs can sit within tau_s of the switch (A6), and as a
+ * brute-force count of the contacts a spatial search must find.
+ */
+void orc_contact_list(int64_t n, const double *x, const double *v, const int32_t *star,
+                      const double *R, int64_t nrows, const int64_t *rows, int64_t cap,
+                      int64_t *count, int64_t *jj, double *rr, double *rd)
+{
+    const int64_t nr = rows ? nrows : n;
+#pragma omp parallel for schedule(static)
+    for (int64_t k = 0; k < nr; ++k) {
+        const int64_t i = rows ? rows[k] : k;
+        int64_t c = 0;
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            const double dx = x[3 * j + 0] - x[3 * i + 0];
+            const double dy = x[3 * j + 1] - x[3 * i + 1];
+            const double dz = x[3 * j + 2] - x[3 * i + 2];
+            const double r = sqrt(dx * dx + dy * dy + dz * dz);
+            if (r == 0.0 || !(r < R[star[i]] + R[star[j]])) continue;
+            if (c < cap) {
+                jj[k * cap + c] = j;
+                rr[k * cap + c] = r;
+                rd[k * cap + c] = (dx * (v[3 * j + 0] - v[3 * i + 0])
+                                 + dy * (v[3 * j + 1] - v[3 * i + 1])
+                                 + dz * (v[3 * j + 2] - v[3 * i + 2])) / r;
+            }
+            ++c;
+        }
+        count[k] = c;
+    }
+}
+
 /* Expanding-star rule (A8): element radius of each star at step n. */
 void orc_radii(int64_t nstep, const double *R_start, const double *R_end,
                int64_t n_ramp, double *R)

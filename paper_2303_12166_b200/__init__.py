@@ -19,7 +19,7 @@ NB_OK, NB_EINVAL, NB_ESTATE, NB_ECUDA, NB_ENOMEM, NB_EARCH = 0, -1, -2, -3, -4, 
 NB_PATH_AUTO, NB_PATH_ONE_SIDED, NB_PATH_SYMMETRIC = 0, 1, 2
 
 EXPORTS = ("nb_create", "nb_workspace_bytes", "nb_set_state", "nb_compute_accel", "nb_step",
-           "nb_energy", "nb_relax", "nb_transfer_diagnostics", "nb_splat", "nb_get_step", "nb_upload_state",
+           "nb_energy", "nb_set_step", "nb_relax", "nb_transfer_diagnostics", "nb_splat", "nb_get_step", "nb_upload_state",
            "nb_download_state",
            "nb_get_launch_info", "nb_set_force_path", "nb_force_kernel_name", "nb_launch_count",
            "nb_time_force_kernel", "nb_time_contact_pass", "nb_destroy", "nb_strerror",
@@ -68,6 +68,8 @@ def lib() -> C.CDLL:
         L.nb_step.argtypes = [vp, C.c_int]
         L.nb_energy.restype = C.c_int
         L.nb_energy.argtypes = [vp, C.POINTER(C.c_double)]
+        L.nb_set_step.restype = C.c_int
+        L.nb_set_step.argtypes = [vp, i64]
         L.nb_relax.restype = C.c_int
         L.nb_relax.argtypes = [vp, C.c_int, C.c_float]
         L.nb_transfer_diagnostics.restype = C.c_int
@@ -169,6 +171,10 @@ def nb_energy(ctx: int) -> Dict[str, object]:
     _check(lib().nb_energy(ctx, out), "nb_energy", ctx)
     v = list(out)
     return dict(KE=v[0], Ug=v[1], Urep=v[2], E=v[3], P=v[4:7], L=v[7:10], Fnet=v[10], step=int(v[11]))
+
+
+def nb_set_step(ctx: int, step: int) -> None:
+    _check(lib().nb_set_step(ctx, int(step)), "nb_set_step", ctx)
 
 
 def nb_relax(ctx: int, nsteps: int, kappa: float) -> None:

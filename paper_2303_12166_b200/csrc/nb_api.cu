@@ -625,6 +625,16 @@ int nb_get_step(nb_ctx* c, int64_t* step, float* R)
     return NB_OK;
 }
 
+int nb_set_step(nb_ctx* c, int64_t step)
+{
+    if (!c || step < 0) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    nb_set_step_kernel<<<1, 1, 0, c->stream>>>(c->dev(), (long long)step);
+    c->launches++;
+    NB_CUDA(c, cudaGetLastError());
+    return NB_OK;
+}
+
 int nb_energy(nb_ctx* c, double* out)
 {
     if (!c || !out) return NB_EINVAL;

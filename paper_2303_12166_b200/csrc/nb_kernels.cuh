@@ -896,6 +896,23 @@ struct UpdateArgs {
     int advance;
 };
 
+// Expanding-star rule (A8): step count n and R_s(n), linear in n over n_ramp steps, evaluated
+// in fp64 with explicit roundings (no contraction) and rounded once to the fp32 model parameter.
+__device__ __forceinline__ void set_step(DevState* d, long long nstep)
+{
+    d->step = nstep;
+    for (int s = 0; s < 2; ++s) {
+        double Rs = d->R_start[s];
+        if (d->n_ramp > 0) {
+            const long long nn = nstep < d->n_ramp ? nstep : d->n_ramp;
+            Rs = __dadd_rn(d->R_start[s],
+                           __ddiv_rn(__dmul_rn(__dsub_rn(d->R_end[s], d->R_start[s]), (double)nn),
+                                     (double)d->n_ramp));
+        }
+        d->R[s] = (float)Rs;
+    }
+}
+
 __global__ void __launch_bounds__(256)
 nb_reduce_update_kernel(const __grid_constant__ UpdateArgs u)
 {
@@ -924,22 +941,11 @@ nb_reduce_update_kernel(const __grid_constant__ UpdateArgs u)
             }
         }
     }
-    if (u.advance && blockIdx.x == 0 && threadIdx.x == 0) {
-        DevState* d = u.dev;
-        const long long nstep = d->step + 1;
-        d->step = nstep;
-        for (int s = 0; s < 2; ++s) {
-            double Rs = d->R_start[s];
-            if (d->n_ramp > 0) {
-                const long long nn = nstep < d->n_ramp ? nstep : d->n_ramp;
-                Rs = __dadd_rn(d->R_start[s],
-                               __ddiv_rn(__dmul_rn(__dsub_rn(d->R_end[s], d->R_start[s]), (double)nn),
-                                         (double)d->n_ramp));
-            }
-            d->R[s] = (float)Rs;
-        }
-    }
+    if (u.advance && blockIdx.x == 0 && threadIdx.x == 0) set_step(u.dev, u.dev->step + 1);
 }
+
+// nb_set_step(): restore the step count of a checkpointed run; the radii follow from it.
+__global__ void nb_set_step_kernel(DevState* dev, long long step) { set_step(dev, step); }
 
 // star[] must be 0...0 1...1; counts the zeros into dev->n1, flags violations.
 __global__ void nb_validate_star_kernel(const int32_t* __restrict__ star, int n, DevState* dev)

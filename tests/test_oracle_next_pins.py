@@ -184,3 +184,55 @@ def test_splat_matches_histogram_away_from_pixel_edges_and_shifts_exactly():
     # moving the window by exactly one pixel (0.0625, a power of two) moves the image by one pixel
     img2 = oracle.splat(pos, star, [0.0625, 0.0, 0.0], 2.0, 0, 2, W, H)
     assert np.array_equal(img2[:, :, :-1], img[:, :, 1:])
+
+
+def test_splat_exact_hand_example_and_ambiguous_band():
+    # the same window as test_splat_hand_example: 8 x 8 pixels of 0.5, x in [-1, 3), y in [0, 4)
+    pos = np.array([[-1.0, 0.0, 9.0], [2.9, 3.9, 0.0], [1.0, 2.0, 0.0], [1.2, 2.4, 5.0], [3.0, 2.0, 0.0], [0.0, -0.1, 0.0]])
+    star = np.array([0, 0, 1, 1, 1, 0])
+    img, amb = oracle.splat_exact(pos, star, [1.0, 2.0, 0.0], 2.0, 0, 1, 8, 8)
+    assert img.dtype == np.uint32 and img.shape == (2, 8, 8) and amb.shape == (2, 10, 10)
+    assert img[0, 0, 0] == 1 and img[0, 7, 7] == 1 and img[1, 4, 4] == 2 and img.sum() == 4
+    # elements exactly on a pixel edge are ambiguous: (-1, 0) -> corner of pixel (0,0); (1, 2) -> corner of (4,4);
+    # (3, 2) -> one pixel right of the window (padded index 8+1); (0, -0.1) -> x on the edge of column 2, one row
+    # below the window (padded row 0); the other two are well inside their pixels
+    assert amb[0, 0 + 1, 0 + 1] == 1 and amb[1, 4 + 1, 4 + 1] == 1 and amb[1, 4 + 1, 8 + 1] == 1
+    assert amb[0, -1 + 1, 2 + 1] == 1 and amb.sum() == 4
+    # the band is 3 W 2^-24 pixels: 8 pixels -> 1.43e-6 pixel = 7.2e-7 length units here
+    eps_in, eps_out = 0.5 * 1.0e-6, 0.5 * 2.0e-6
+    pos = np.array([[0.5 + eps_in, 1.25, 0.0], [0.5 - eps_in, 1.25, 0.0], [0.5 + eps_out, 1.25, 0.0]])
+    img, amb = oracle.splat_exact(pos, np.zeros(3, int), [1.0, 2.0, 0.0], 2.0, 0, 1, 8, 8)
+    assert img[0, 2, 3] == 2 and img[0, 2, 2] == 1             # decided exactly, whichever side
+    assert amb[0, 2 + 1, 3 + 1] == 1 and amb[0, 2 + 1, 2 + 1] == 1 and amb.sum() == 2
+
+
+def test_splat_exact_is_the_histogram_and_the_float32_recipe_agrees_off_the_band():
+    rng = np.random.default_rng(8)
+    W, H = 96, 64
+    pos = rng.uniform(-2.2, 2.2, (20000, 3)).astype(np.float32)
+    star = (rng.uniform(size=len(pos)) < 0.4).astype(np.int32)
+    c, hw = [0.125, 0.0, -0.25], 2.0
+    img, amb = oracle.splat_exact(pos, star, c, hw, 0, 2, W, H)
+    half_v = hw * H / W
+    for s in (0, 1):
+        q = pos[star == s].astype(np.float64)
+        # numpy's own binning of the same window (its last bin is closed on the right: no point sits there)
+        h, _, _ = np.histogram2d(q[:, 2], q[:, 0], bins=[H, W],
+                                 range=[[c[2] - half_v, c[2] + half_v], [c[0] - hw, c[0] + hw]])
+        assert np.array_equal(img[s], h.astype(np.uint32))
+    assert 0 < img.sum() < len(pos)
+    # the float32 recipe (what the kernel computes) differs from the definition only through ambiguous elements:
+    # per pixel, by no more than the ambiguous elements of its 3 x 3 neighbourhood
+    f32 = oracle.splat(pos, star, c, hw, 0, 2, W, H).astype(np.int64)
+    nb_amb = sum(amb[:, 1 + dy:1 + dy + H, 1 + dx:1 + dx + W].astype(np.int64) for dy in (-1, 0, 1) for dx in (-1, 0, 1))
+    assert (np.abs(f32 - img.astype(np.int64)) <= nb_amb).all()
+    # with points placed on purpose a hair around pixel edges the two may differ, but only inside that allowance
+    edge = np.zeros((4000, 3), np.float32)
+    k = rng.integers(0, W, 4000)
+    edge[:, 0] = (c[0] - hw + k * (2 * hw / W) + rng.uniform(-3e-7, 3e-7, 4000)).astype(np.float32)
+    edge[:, 2] = rng.uniform(-1.0, 1.0, 4000).astype(np.float32)
+    img, amb = oracle.splat_exact(edge, np.zeros(4000, int), c, hw, 0, 2, W, H)
+    f32 = oracle.splat(edge, np.zeros(4000, int), c, hw, 0, 2, W, H).astype(np.int64)
+    nb_amb = sum(amb[:, 1 + dy:1 + dy + H, 1 + dx:1 + dx + W].astype(np.int64) for dy in (-1, 0, 1) for dx in (-1, 0, 1))
+    assert amb.sum() > 1000 and (np.abs(f32 - img.astype(np.int64)) <= nb_amb).all()
+    assert abs(int(f32.sum()) - int(img.sum())) <= int(amb[:, :, [0, 1, W, W + 1]].sum() + amb[:, [0, 1, H, H + 1], :].sum())

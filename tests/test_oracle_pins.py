@@ -417,3 +417,134 @@ def test_rows_subset_and_thread_count_independence():
     rows = np.array([5, 0, 300, 511])
     ar = oracle.accel(w.posm, w.vel, m, w.star, w.params["R_start"], w.params, rows=rows)
     assert np.array_equal(a[rows], ar)
+
+
+# ------------------------- A6: the allowance every parity assertion subtracts (orc_accel's delta)
+def test_a6_delta_hand_numbers_band_and_branch_independence():
+    # geometry of test_contact_hand_numbers_and_branch: R = 1, r = 1 -> pi V = 5 pi/12 = 1.308996939,
+    # gamma = 3, beta = 0.25, m = (2, 5), rdot = -0.2.  A pair within tau_s of the switch contributes
+    # (1 - beta) gamma pi V / m_i:  0.75 * 3 * 1.308996939 / 2 = 1.472621556,  / 5 = 0.589048623.
+    x = [[0, 0, 0], [1, 0, 0]]
+    v = [[0.1, 0, 0], [-0.1, 0, 0]]
+    kw = dict(P0, G=0.0, gamma=3.0, beta=0.25)
+
+    def delta(**over):
+        a, kap, dl = oracle.accel(np.array(x, float), np.array(over.pop("v", v), float), np.array([2.0, 5.0]),
+                                  np.zeros(2, np.int32), over.pop("R", (1.0, 1.0)), dict(kw, **over), want_diag=True)
+        return a, dl
+
+    a_lo, dl = delta(v_dead=0.2 - 5e-6, tau_s=1e-5)          # |rdot + v_dead| = 5e-6 <= tau_s
+    assert dl == pytest.approx([1.472621556, 0.589048623], abs=1e-9)
+    a_hi, dl2 = delta(v_dead=0.2 + 5e-6, tau_s=1e-5)         # the other side of the switch: same allowance
+    assert np.array_equal(dl, dl2)
+    # ... and the two sides differ by exactly that allowance (gamma vs gamma*beta on the one pair)
+    assert np.abs(a_lo - a_hi)[:, 0] == pytest.approx(dl, rel=1e-12)
+    assert delta(v_dead=0.2 - 5e-6, tau_s=1e-6)[1] == pytest.approx([0.0, 0.0], abs=0)    # outside the band
+    assert delta(v_dead=0.2 + 5e-6, tau_s=4.9e-6)[1] == pytest.approx([0.0, 0.0], abs=0)
+    assert delta(v_dead=0.2 + 5e-6, tau_s=5.1e-6)[1][0] > 0                                # band edge is 5e-6
+    assert delta(v_dead=0.0, tau_s=1e-5)[1] == pytest.approx([0.0, 0.0], abs=0)            # rdot = -0.2 is far from 0
+    # the band is |rdot + v_dead|, in velocity units, symmetric: rdot = +0.2 (diverging) with v_dead = 0 is far, too
+    assert delta(v=[[-0.1, 0, 0], [0.1, 0, 0]], v_dead=0.0, tau_s=0.19)[1] == pytest.approx([0.0, 0.0], abs=0)
+    assert delta(v=[[-0.1, 0, 0], [0.1, 0, 0]], v_dead=0.0, tau_s=0.21)[1][0] == pytest.approx(1.472621556, abs=1e-9)
+    # a pair that is not in contact has no allowance, whatever its rdot
+    x[1][0] = 2.0
+    assert delta(v_dead=0.2, tau_s=1.0)[1] == pytest.approx([0.0, 0.0], abs=0)
+    x[1][0] = 1.0
+    # gamma = 0 (no contact terms at all) and beta = 1 (both branches equal): nothing to allow for
+    assert delta(v_dead=0.2, tau_s=1.0, gamma=0.0)[1] == pytest.approx([0.0, 0.0], abs=0)
+    assert delta(v_dead=0.2, tau_s=1.0, beta=1.0)[1] == pytest.approx([0.0, 0.0], abs=0)
+
+
+def test_a6_delta_sums_over_the_ambiguous_pairs_of_a_row_only():
+    # element 0 touches 1 (on the switch) and 2 (clearly converging): only pair (0,1) is allowed for.
+    # R = 1: pair (0,1) r = 1 -> pi V = 5 pi/12; pair (0,2) r = 1.5 -> pi (0.5)^2 (5.5)/12 = 0.359974158
+    x = np.array([[0, 0, 0], [1, 0, 0], [-1.5, 0, 0]], float)           # 1 and 2 are 2.5 apart: no contact
+    v = np.array([[0, 0, 0], [-0.2, 0, 0], [3.0, 0, 0]], float)
+    p = dict(P0, G=0.0, gamma=2.0, beta=0.5, v_dead=0.2, tau_s=1e-9)
+    a, kap, dl = oracle.accel(x, v, np.array([1.0, 1.0, 4.0]), np.zeros(3, np.int32), (1.0, 1.0), p, want_diag=True)
+    assert dl == pytest.approx([0.5 * 2.0 * 1.308996939, 0.5 * 2.0 * 1.308996939, 0.0], abs=1e-9)
+    # rdot == -v_dead exactly is NOT converging (A5: strict <): pair (0,1) takes gamma*beta, pair (0,2) gamma
+    assert a[0] == pytest.approx([-1.0 * 1.308996939 + 2.0 * 0.359974158, 0.0, 0.0], abs=1e-9)
+    assert a[2] == pytest.approx([-2.0 * 0.359974158 / 4.0, 0.0, 0.0], abs=1e-9)
+
+
+def test_kappa_hand_values():
+    # kappa_i = sum_j |a_ij| / |a_i|.  Two bodies: one term, kappa = 1 exactly.
+    a, kap, dl = oracle.accel(np.array([[0, 0, 0], [3.0, 0, 0]]), np.zeros((2, 3)), np.array([1.0, 2.0]),
+                              np.zeros(2, np.int32), (0, 0), dict(P0, eps=1.0), want_diag=True)
+    assert kap == pytest.approx([1.0, 1.0], abs=1e-15) and (dl == 0).all()
+    # the collinear case of test_p1_collinear_unequal_masses_literal: the middle element is pulled both ways,
+    # kappa_1 = (0.888888889 + 1.28) / 0.391111111 = 5.545454545; the outer ones one way only
+    a, kap, _ = oracle.accel(np.array([[0, 0, 0], [1.0, 0, 0], [3.0, 0, 0]]), np.zeros((3, 3)),
+                             np.array([1.0, 2.0, 4.0]), np.zeros(3, np.int32), (0, 0), dict(P0, G=2.0, eps=0.5),
+                             want_diag=True)
+    assert kap == pytest.approx([1.0, 5.545454545, 1.0], abs=2e-9)
+    # a contact term counts with its own magnitude: gravity 1/(1+0)^2 = 1 toward j, repulsion 3 * 5pi/12 / 2 away
+    a, kap, _ = oracle.accel(np.array([[0, 0, 0], [1.0, 0, 0]]), np.array([[0.1, 0, 0], [-0.1, 0, 0]]),
+                             np.array([2.0, 1.0]), np.zeros(2, np.int32), (1.0, 1.0),
+                             dict(P0, G=1.0, gamma=3.0, beta=0.25), want_diag=True)
+    assert a[0, 0] == pytest.approx(1.0 - 1.963495408, abs=1e-9) and kap[0] == pytest.approx(1.0, abs=1e-12)
+
+
+def test_energy_net_force_output_hand_pair():
+    # out[10] = |sum_i m_i a_i| of the acceleration array handed in: m = (2, 3), a = ((1,0,0), (0,2,0))
+    # -> |(2, 6, 0)| = sqrt(40) = 6.32455532
+    posm = np.array([[0, 0, 0, 2.0], [0, 4, 0, 3.0]], np.float32)
+    s = oracle.Sim(posm, np.zeros((2, 4), np.float32), np.zeros(2, np.int32),
+                   dict(P0, eps=1.0, dt=1.0, R_start=(0, 0), R_end=(0, 0), n_ramp=0))
+    s.acc[:] = [[1.0, 0, 0], [0, 2.0, 0]]
+    s.have_acc.value = 1
+    assert s.energy()["Fnet"] == pytest.approx(6.32455532, abs=1e-8)
+    s.have_acc.value = 0                      # computed from the state: Newton's third law, exactly opposite forces
+    assert s.energy()["Fnet"] == pytest.approx(0.0, abs=1e-15)
+
+
+def test_contact_list_hand_and_brute_force():
+    # hand pair of the tests above: r = 1, rdot = -0.2, seen from both sides; a third element out of reach
+    x = np.array([[0, 0, 0], [1, 0, 0], [0, 2.5, 0]], float)
+    v = np.array([[0.1, 0, 0], [-0.1, 0, 0], [0, 0, 0]], float)
+    cnt, jj, rr, rd = oracle.contact_list(x, v, np.array([0, 0, 1], np.int32), (1.0, 1.0))
+    assert cnt.tolist() == [1, 1, 0] and jj[:, 0].tolist() == [1, 0, -1]
+    assert rr[:2, 0] == pytest.approx([1.0, 1.0]) and rd[:2, 0] == pytest.approx([-0.2, -0.2], abs=1e-15)
+    # A2: cross-star reach is R_0 + R_1 = 1.6 < 2.5; with R_1 = 2 element 2 touches 0 (r = 2.5 < 3) but sideways: rdot = 0...
+    cnt, jj, rr, rd = oracle.contact_list(x, v, np.array([0, 0, 1], np.int32), (1.0, 2.0), rows=[2, 0])
+    assert cnt.tolist() == [2, 2] and jj[0, :2].tolist() == [0, 1] and jj[1, :2].tolist() == [1, 2]
+    assert rr[0, 0] == pytest.approx(2.5) and rd[0, 0] == pytest.approx(0.0, abs=1e-15)
+    # ... and moving toward it along the line of centres: rdot = -speed, the same seen from either element
+    v[2] = [0, -0.7, 0]
+    assert oracle.contact_list(x, v, np.array([0, 0, 1], np.int32), (1.0, 2.0), rows=[2])[3][0, 0] == pytest.approx(-0.7)
+    assert oracle.contact_list(x, v, np.array([0, 0, 1], np.int32), (1.0, 2.0), rows=[0])[3][0, 1] == pytest.approx(-0.7)
+    # brute force on a seeded workload, with numpy: same counts, same partners, same rdot; cap truncates the lists only
+    w = make_binary(name="t", seed=9, n1=200, n2=150, shape="uniform", radius1=1.0, radius2=0.6, q=0.5, a=1.4,
+                    eps=0.01, dt=1e-3, nsteps=0)
+    R = np.array(w.params["R_start"])
+    X, V = w.posm[:, :3].astype(float), w.vel[:, :3].astype(float)
+    cnt, jj, rr, rd = oracle.contact_list(X, V, w.star, R, cap=6)
+    d = X[None, :, :] - X[:, None, :]
+    r = np.sqrt((d ** 2).sum(-1))
+    reach = R[w.star][:, None] + R[w.star][None, :]
+    touch = (r < reach) & (r > 0)
+    assert np.array_equal(cnt, touch.sum(1)) and cnt.max() > 6 and (cnt == 0).any()
+    rdot = (d * (V[None, :, :] - V[:, None, :])).sum(-1) / np.where(r > 0, r, 1.0)
+    for i in range(w.n):
+        js = np.flatnonzero(touch[i])[:6]
+        assert jj[i, :len(js)].tolist() == js.tolist() and (jj[i, len(js):] == -1).all()
+        assert np.allclose(rd[i, :len(js)], rdot[i, js], rtol=1e-13, atol=1e-15)
+    # the contact terms of orc_accel act on exactly these rows
+    p = dict(w.params, R_start=tuple(R))
+    a1 = oracle.accel(w.posm, w.vel, w.posm[:, 3], w.star, R, p)
+    a0 = oracle.accel(w.posm, w.vel, w.posm[:, 3], w.star, R, dict(p, gamma=0.0))
+    assert np.array_equal(np.linalg.norm(a1 - a0, axis=1) > 0, cnt > 0)
+
+
+def test_a6_population_follows_from_the_rdot_density(small_binary):
+    """The number of rows with delta > 0 is what the rdot distribution of the contact pairs predicts:
+    pairs within tau_s of -v_dead.  (The GPU tests bound their A6 population the same way.)"""
+    w = small_binary
+    R = np.array(w.params["R_start"]) * 1.5
+    p = dict(w.params, tau_s=0.02 * w.meta["omega"] * w.meta["a"])      # a wide band so that it is populated
+    _, _, dl = oracle.accel(w.posm, w.vel, w.posm[:, 3], w.star, R, p, want_diag=True)
+    cnt, jj, rr, rd = oracle.contact_list(w.posm, w.vel, w.star, R, cap=int(64))
+    assert cnt.max() <= 64
+    inband = np.abs(rd + p["v_dead"]) <= p["tau_s"]                      # NaN (no pair) compares False
+    assert np.array_equal(dl > 0, inband.any(1)) and 3 < (dl > 0).sum() < w.n
