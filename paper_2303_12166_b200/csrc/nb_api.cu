@@ -3,8 +3,7 @@
 // arithmetic step of the path runs in the kernels of nb_kernels.cuh.
 #include "nb.h"
 #include "nb_kernels.cuh"
-
-#include <cub/device/device_radix_sort.cuh>   // CUDA-toolkit radix sort: orders (Hilbert key, index) pairs only
+#include "nb_cells.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -35,9 +34,9 @@ struct Plan {           // launch configuration of the gravity kernel for a give
 constexpr int kCtasPerSM = 8;                      // resident CTAs/SM of nb_gravity_kernel<2, .> (64 registers)
 constexpr int64_t kMaxSplit = 64;
 constexpr int64_t kPartialBudget = (int64_t)128 << 20;   // bytes of split-j partial sums worth keeping in L2
-constexpr int64_t kSortMinN = 8192;                // below this the contact pass takes groups in index order
-constexpr int64_t kContactWarps = 4096;            // warps wanted in flight by the contact kernel
-constexpr int kMaxContactChunks = 32;              // ... and splits the candidate groups of a warp into this many slabs
+constexpr int64_t kCellMinN = 8192;                // below this the contact pass takes groups in index order (all pairs
+                                                   // pre-tested), from here on it builds the cell list
+constexpr int kMaxContactChunks = 32;              // index-order search: the candidate groups of a warp go to this many slabs
 
 // Force-path selection (nb_set_force_path).
 enum { kPathAuto = 0, kPathOneSided = 1, kPathSymmetric = 2 };
@@ -60,17 +59,22 @@ int sym_tile(int64_t n)
 
 int64_t sym_slabs(int64_t n) { const int64_t S = sym_tile(n); return (n + S - 1) / S; }
 
-// Slabs the contact pass writes for n elements: one per chunk of candidate groups (index order,
-// n < kSortMinN) or per round-robin share of the candidate groups (sorted search) that a warp takes.
+// Slabs the contact pass writes for n elements: one (cell list), or one per chunk of candidate groups
+// (index-order search, n < kCellMinN).
 int contact_slabs(int64_t n)
 {
+    if (n >= kCellMinN) return 1;
     const int64_t ngroups = (n + kGroup - 1) / kGroup;
-    if (n < kSortMinN) return (int)(ngroups < kMaxContactChunks ? ngroups : kMaxContactChunks);
-    const int64_t nsuper = (ngroups + kSuper - 1) / kSuper;
-    int64_t ch = kContactWarps / ngroups;          // enough warps to fill the machine
-    if (ch > nsuper) ch = nsuper;
-    if (ch > kMaxContactChunks) ch = kMaxContactChunks;
-    return (int)(ch < 1 ? 1 : ch);
+    return (int)(ngroups < kMaxContactChunks ? ngroups : kMaxContactChunks);
+}
+
+// Buckets of the cell table of a star of ns elements: a power of two in [2 ns, 4 ns), at least 64 (4 x 4 x 4).
+int64_t cell_cap(int64_t ns)
+{
+    if (ns <= 0) return 0;
+    int64_t c = 64;
+    while (c < 2 * ns) c <<= 1;
+    return c;
 }
 
 // Largest number of j splits allowed for n elements (bounds the partial-sum slabs).
@@ -131,12 +135,12 @@ Plan make_plan(int64_t n, int num_sms, int path)
 }
 
 struct Layout {
-    size_t off_dev, off_acc, off_part, off_red, off_keys, off_vals, off_sorttmp, off_ps, off_vs, off_gbox,
-        off_sbox, off_boxes, total;
-    size_t sorttmp_bytes;
+    size_t off_dev, off_acc, off_part, off_red, off_ps, off_vs, off_gbox, off_sbox, off_cpart, off_cstate,
+        off_counters, off_bsum, off_bucket, off_slot, off_tmp, off_perm, total;
 };
 
-size_t sort_temp_bound(int64_t n_max) { return (size_t)n_max * 16 + ((size_t)8 << 20); }
+// cell_cap(n1) + cell_cap(n - n1) < 4 n + 128 for every split of n <= n_max elements
+int64_t cell_counters_bound(int64_t n_max) { return 4 * n_max + 129; }
 
 Layout make_layout(int64_t n_max)
 {
@@ -150,15 +154,19 @@ Layout make_layout(int64_t n_max)
     const size_t pot_blocks = (size_t)((n_max + kThreads - 1) / kThreads);
     const size_t red = (size_t)kMomentBlocks * 16 * sizeof(double) + pot_blocks * 2 * sizeof(double);   // 16 >= kMomentCols, kXferCols1, kXferCols2
     L.off_red = o;  o += align_up(red);
-    L.off_keys = o; o += align_up((size_t)n_max * 2 * sizeof(unsigned long long));   // key double buffer
-    L.off_vals = o; o += align_up((size_t)n_max * 2 * sizeof(uint32_t));             // index double buffer
-    L.sorttmp_bytes = sort_temp_bound(n_max);
-    L.off_sorttmp = o; o += align_up(L.sorttmp_bytes);
     L.off_ps = o;   o += align_up((size_t)n_max * sizeof(float4));
     L.off_vs = o;   o += align_up((size_t)n_max * sizeof(float4));
     L.off_gbox = o; o += align_up(ngroups * 2 * sizeof(float4));
     L.off_sbox = o; o += align_up(nsuper * 2 * sizeof(float4));
-    L.off_boxes = o; o += align_up((size_t)kBoxBlocks * 2 * sizeof(float4));
+    const size_t ncnt = (size_t)cell_counters_bound(n_max);
+    L.off_cpart = o;    o += align_up((size_t)kBoxBlocks * 2 * sizeof(CellPartial));
+    L.off_cstate = o;   o += align_up(sizeof(CellState));
+    L.off_counters = o; o += align_up(ncnt * sizeof(int));
+    L.off_bsum = o;     o += align_up((ncnt / kCellScanChunk + 2) * sizeof(int));
+    L.off_bucket = o;   o += align_up((size_t)n_max * sizeof(int));
+    L.off_slot = o;     o += align_up((size_t)n_max * sizeof(int));
+    L.off_tmp = o;      o += align_up((size_t)n_max * sizeof(int));
+    L.off_perm = o;     o += align_up((size_t)n_max * sizeof(uint32_t));
     L.total = o;
     return L;
 }
@@ -187,13 +195,11 @@ struct nb_ctx {
     float4* acc() const { return reinterpret_cast<float4*>(ws + lay.off_acc); }
     float4* part() const { return reinterpret_cast<float4*>(ws + lay.off_part); }
     double* red() const { return reinterpret_cast<double*>(ws + lay.off_red); }
-    unsigned long long* keys() const { return reinterpret_cast<unsigned long long*>(ws + lay.off_keys); }
-    uint32_t* vals() const { return reinterpret_cast<uint32_t*>(ws + lay.off_vals); }
     float4* ps() const { return reinterpret_cast<float4*>(ws + lay.off_ps); }
     float4* vs() const { return reinterpret_cast<float4*>(ws + lay.off_vs); }
     float4* gbox() const { return reinterpret_cast<float4*>(ws + lay.off_gbox); }
     float4* sbox() const { return reinterpret_cast<float4*>(ws + lay.off_sbox); }
-    float4* boxes() const { return reinterpret_cast<float4*>(ws + lay.off_boxes); }
+    template <class T> T* at(size_t off) const { return reinterpret_cast<T*>(ws + off); }
     bool contact_on() const { return prm.gamma > 0.f; }
     int ngrav() const { return plan.sym_S ? plan.T : plan.nsplit; }       // gravity slabs
     int ncontact() const {                                                // contact slabs
@@ -269,48 +275,55 @@ int launch_gravity(nb_ctx* c)
     return NB_OK;
 }
 
-// Row a3: contact accelerations (Eqs. 5/6) of the pairs with r < R_i + R_j -> part[P][n]
+// Row a3: contact accelerations (Eqs. 5/6) of the pairs with r < R_i + R_j -> part[ngrav ...][n]
 int launch_contact_on(nb_ctx* c, cudaStream_t st)
 {
     const int n = (int)c->n;
-    const uint32_t* perm = nullptr;
-    if (c->n >= kSortMinN) {
-        nb_bbox_kernel<<<kBoxBlocks, 256, 0, st>>>(c->posm, n, c->boxes());
-        c->launches++;
-        // cells per axis: ~16 per mean element spacing is plenty to order elements into compact groups, and
-        // every 8 key bits less is one pass less of the radix sort (n = 65,536: 30 bits, 4 passes instead of 6)
-        int bits = 4;
-        while ((1ll << (3 * (bits - 4))) < c->n && bits < kKeyBits) ++bits;
-        nb_keys_kernel<<<(n + 255) / 256, 256, 0, st>>>(c->posm, n, c->boxes(), c->keys(), c->vals(), bits);
-        c->launches++;
-        NB_CUDA(c, cudaGetLastError());
-        cub::DoubleBuffer<unsigned long long> dk(c->keys(), c->keys() + c->n_max);
-        cub::DoubleBuffer<uint32_t> dv(c->vals(), c->vals() + c->n_max);
-        size_t tmp = c->lay.sorttmp_bytes;
-        NB_CUDA(c, cub::DeviceRadixSort::SortPairs(c->ws + c->lay.off_sorttmp, tmp, dk, dv, n, 0, 3 * bits, st));
-        c->launches += 1;                              // counted as one (library) launch
-        perm = dv.Current();
-    }
-    const int ngroups = (n + kGroup - 1) / kGroup;
-    const int nsuper = (ngroups + kSuper - 1) / kSuper;
-    nb_gather_kernel<<<nsuper, kGroup * kSuper, 0, st>>>(c->posm, c->vel, perm, n, c->dev(), c->ps(), c->vs(),
-                                                               c->gbox(), c->sbox());
-    c->launches++;
     ContactArgs ca;
-    ca.ps = c->ps(); ca.vs = c->vs(); ca.perm = perm; ca.gbox = c->gbox(); ca.sbox = c->sbox();
+    ca.ps = c->ps(); ca.vs = c->vs(); ca.perm = nullptr; ca.gbox = c->gbox(); ca.sbox = c->sbox();
     ca.out = c->part() + (size_t)c->ngrav() * c->n;
-    ca.n = n; ca.ngroups = ngroups; ca.nsuper = nsuper;
+    ca.n = n;
     ca.gamma = c->prm.gamma; ca.gamma_beta = c->prm.gamma * c->prm.beta;
     ca.v_dead = c->prm.v_dead; ca.lens_mode = c->prm.lens_mode;
+    if (c->n >= kCellMinN) {                                      // cell list (nb_cells.cuh)
+        const Layout& L = c->lay;
+        CellArgs a;
+        a.posm = c->posm; a.vel = c->vel; a.dev = c->dev();
+        a.part = c->at<CellPartial>(L.off_cpart); a.cs = c->at<CellState>(L.off_cstate);
+        a.counters = c->at<int>(L.off_counters); a.bsum = c->at<int>(L.off_bsum);
+        a.bucket = c->at<int>(L.off_bucket); a.slot = c->at<int>(L.off_slot); a.tmp = c->at<int>(L.off_tmp);
+        a.perm = c->at<uint32_t>(L.off_perm); a.ps = c->ps(); a.vs = c->vs();
+        a.n = n; a.n1 = c->n1;
+        a.cap0 = (int)cell_cap(c->n1); a.cap1 = (int)cell_cap(c->n - c->n1); a.ncells = a.cap0 + a.cap1;
+        const int eb = (n + 255) / 256;
+        const int sb = (a.ncells + kCellScanChunk - 1) / kCellScanChunk;
+        nb_cell_bbox_kernel<<<kBoxBlocks, 256, 0, st>>>(c->posm, n, c->n1, c->at<CellPartial>(L.off_cpart), a.counters,
+                                                       a.ncells + 1);
+        nb_cell_count_kernel<<<eb, 256, 0, st>>>(a);
+        if (sb > 1) { nb_cell_scan_kernel<<<sb, 1024, 0, st>>>(a.counters, a.bsum, a.ncells, 0); c->launches++; }
+        nb_cell_scan_kernel<<<sb, 1024, 0, st>>>(a.counters, a.bsum, a.ncells, 1);
+        nb_cell_scatter_kernel<<<eb, 256, 0, st>>>(a);
+        nb_cell_rank_kernel<<<eb, 256, 0, st>>>(a);
+        CellContactArgs k;
+        k.ps = c->ps(); k.vs = c->vs(); k.perm = a.perm; k.start = a.counters; k.cs = a.cs; k.dev = c->dev();
+        k.out = ca.out; k.law = ca; k.n = n;
+        nb_contact_cell_kernel<<<(n + kThreads - 1) / kThreads, kThreads, 0, st>>>(k);
+        c->launches += 6;
+        NB_CUDA(c, cudaGetLastError());
+        return NB_OK;
+    }
+    // small n: groups of 32 in index order, every group a candidate of every other
+    const int ngroups = (n + kGroup - 1) / kGroup;
+    const int nsuper = (ngroups + kSuper - 1) / kSuper;
+    nb_gather_kernel<<<nsuper, kGroup * kSuper, 0, st>>>(c->posm, c->vel, nullptr, n, c->dev(), c->ps(), c->vs(),
+                                                               c->gbox(), c->sbox());
+    c->launches++;
+    ca.ngroups = ngroups; ca.nsuper = nsuper;
     const int nchunks = c->ncontact();
     const long long warps = (long long)ngroups * nchunks;
     ca.nchunks = nchunks;
-    if (perm) {
-        nb_contact_kernel<<<(int)((warps * 32 + kThreads - 1) / kThreads), kThreads, 0, st>>>(ca);
-    } else {
-        const int cg = (ngroups + nchunks - 1) / nchunks;
-        nb_contact_chunk_kernel<<<(int)((warps * 32 + kThreads - 1) / kThreads), kThreads, 0, st>>>(ca, cg, nchunks);
-    }
+    const int cg = (ngroups + nchunks - 1) / nchunks;
+    nb_contact_chunk_kernel<<<(int)((warps * 32 + kThreads - 1) / kThreads), kThreads, 0, st>>>(ca, cg, nchunks);
     c->launches++;
     NB_CUDA(c, cudaGetLastError());
     return NB_OK;
@@ -418,16 +431,6 @@ int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream
         cudaFuncSetAttribute(NB_SYM_4096, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 4096) != cudaSuccess) {
         nb_destroy(c);
         return NB_ECUDA;
-    }
-    {   // the radix sort's scratch must fit the slice the layout reserves for it
-        size_t need = 0;
-        cub::DoubleBuffer<unsigned long long> dk(nullptr, nullptr);
-        cub::DoubleBuffer<uint32_t> dv(nullptr, nullptr);
-        if (cub::DeviceRadixSort::SortPairs(nullptr, need, dk, dv, (int)n_max, 0, 3 * kKeyBits, c->stream) != cudaSuccess ||
-            need > c->lay.sorttmp_bytes) {
-            nb_destroy(c);
-            return NB_ENOMEM;
-        }
     }
     *out = c;
     return NB_OK;

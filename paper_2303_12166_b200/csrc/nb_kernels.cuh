@@ -483,21 +483,17 @@ nb_gravity_sym_kernel(const __grid_constant__ SymArgs a)
 // ---------------------------------------------------------------------------
 // Row a3: contact repulsion, Eqs. 5/6, for exactly the pairs with
 // r < R_i + R_j.  These are ~5 pairs per element out of N, so they are found by a spatial
-// search instead of a test inside the N^2 loop:
-//   nb_bbox_kernel    bounding box of all elements (block partials, no atomics)
-//   nb_keys_kernel    48-bit Hilbert-curve key of every element inside that box
-//   [radix sort of (key, index) -> perm; host side, nb_api.cu]
-//   nb_gather_kernel  elements in Hilbert order: ps = (x,y,z,R_star), vs = (vx,vy,vz,m);
-//                     bounding box + largest radius of every group of 32 and of every
-//                     super-group of 32 groups
-//   nb_contact_kernel one warp per group of 32 elements i (one per lane): scan the super-group
-//                     boxes, then the group boxes of the near super-groups (box against box), then
-//                     each lane's point against the box of every candidate group, then every j of
-//                     the groups that survive; a pair in contact is evaluated in fp64.
-// The box tests are conservative (a pair in contact is never skipped); which pairs ARE in
-// contact is decided by the fp64 test r < R_i + R_j alone, so the result does not depend on
-// the order.  For small n the sort is skipped (perm == nullptr: groups in index order).
-constexpr int kBoxBlocks = 128;       // partial boxes of nb_bbox_kernel
+// search instead of a test inside the N^2 loop: for n >= 8,192 through the cell list of
+// nb_cells.cuh; for smaller n (where a warp per 32 elements cannot fill the machine anyway) by
+// testing every pair, dealt to many warps:
+//   nb_gather_kernel        ps = (x,y,z,R_star), vs = (vx,vy,vz,m) in index order; bounding box +
+//                           largest radius of every group of 32 elements
+//   nb_contact_chunk_kernel one warp per (group of 32 elements i, chunk of groups j): each lane's
+//                           point against the box of every group of the chunk, then every j of the
+//                           groups that survive; a pair in contact is evaluated in fp64.
+// The box and fp32 tests are conservative (a pair in contact is never skipped); which pairs ARE in
+// contact is decided by the fp64 test r < R_i + R_j alone.
+constexpr int kBoxBlocks = 128;       // blocks (= partial boxes) of nb_cell_bbox_kernel
 constexpr int kGroup = 32;            // elements per group (one warp)
 constexpr int kSuper = 32;            // groups per super-group (one 1024-thread block of the gather)
 
@@ -508,99 +504,6 @@ __device__ __forceinline__ float warp_min(float v) {
 __device__ __forceinline__ float warp_max(float v) {
     for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
     return v;
-}
-
-// boxes[2b] = (lo.xyz, 0), boxes[2b+1] = (hi.xyz, 0) of block b's grid-stride share.
-__global__ void __launch_bounds__(256)
-nb_bbox_kernel(const float4* __restrict__ posm, int n, float4* __restrict__ boxes)
-{
-    __shared__ float sh[6][8];
-    float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
-        const float4 p = posm[i];
-        lo[0] = fminf(lo[0], p.x); lo[1] = fminf(lo[1], p.y); lo[2] = fminf(lo[2], p.z);
-        hi[0] = fmaxf(hi[0], p.x); hi[1] = fmaxf(hi[1], p.y); hi[2] = fmaxf(hi[2], p.z);
-    }
-    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
-    for (int c = 0; c < 3; ++c) {
-        const float a = warp_min(lo[c]), b = warp_max(hi[c]);
-        if (l == 0) { sh[c][w] = a; sh[3 + c][w] = b; }
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int c = 0; c < 3; ++c)
-            for (int k = 1; k < 8; ++k) { sh[c][0] = fminf(sh[c][0], sh[c][k]); sh[3 + c][0] = fmaxf(sh[3 + c][0], sh[3 + c][k]); }
-        boxes[2 * blockIdx.x] = make_float4(sh[0][0], sh[1][0], sh[2][0], 0.f);
-        boxes[2 * blockIdx.x + 1] = make_float4(sh[3][0], sh[4][0], sh[5][0], 0.f);
-    }
-}
-
-// Spread the low 16 bits of v to every third bit.
-__device__ __forceinline__ unsigned long long spread3(unsigned long long v) {
-    v &= 0xffffull;
-    v = (v | (v << 16)) & 0x0000ff0000ffull;
-    v = (v | (v << 8))  & 0x00f00f00f00full;
-    v = (v | (v << 4))  & 0x0c30c30c30c3ull;
-    v = (v | (v << 2))  & 0x249249249249ull;
-    return v;
-}
-
-constexpr int kKeyBits = 16;          // most bits per axis; keys have at most 3*kKeyBits = 48 significant bits
-
-// Index of the cell (qx, qy, qz) along the 3-D Hilbert curve of order `bits` <= kKeyBits (Skilling's
-// axes-to-transpose transform, then bit interleave).  Unlike the Z-order curve it has no
-// jumps, so 32 consecutive elements always form a compact group.
-__device__ __forceinline__ unsigned long long hilbert_key(uint32_t qx, uint32_t qy, uint32_t qz, int bits) {
-    uint32_t X[3] = {qx, qy, qz};
-    for (uint32_t Q = 1u << (bits - 1); Q > 1; Q >>= 1) {
-        const uint32_t P = Q - 1;
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-            if (X[i] & Q) X[0] ^= P;
-            else { const uint32_t t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
-        }
-    }
-    X[1] ^= X[0]; X[2] ^= X[1];
-    uint32_t t = 0;
-    for (uint32_t Q = 1u << (bits - 1); Q > 1; Q >>= 1)
-        if (X[2] & Q) t ^= Q - 1;
-    X[0] ^= t; X[1] ^= t; X[2] ^= t;
-    return (spread3(X[0]) << 2) | (spread3(X[1]) << 1) | spread3(X[2]);
-}
-
-__global__ void __launch_bounds__(256)
-nb_keys_kernel(const float4* __restrict__ posm, int n, const float4* __restrict__ boxes,
-               unsigned long long* __restrict__ keys, uint32_t* __restrict__ vals, int bits)
-{
-    __shared__ float sh[4];
-    const float kCells = (float)((1 << bits) - 1);
-    if (threadIdx.x < 32) {                       // reduce the kBoxBlocks partial boxes (cubic cells)
-        float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
-        for (int b = threadIdx.x; b < kBoxBlocks; b += 32) {
-            const float4 l = boxes[2 * b], h = boxes[2 * b + 1];
-            lo[0] = fminf(lo[0], l.x); lo[1] = fminf(lo[1], l.y); lo[2] = fminf(lo[2], l.z);
-            hi[0] = fmaxf(hi[0], h.x); hi[1] = fmaxf(hi[1], h.y); hi[2] = fmaxf(hi[2], h.z);
-        }
-        float ext = 0.f;
-        for (int c = 0; c < 3; ++c) {
-            lo[c] = warp_min(lo[c]); hi[c] = warp_max(hi[c]);
-            ext = fmaxf(ext, hi[c] - lo[c]);
-        }
-        if (threadIdx.x == 0) {
-            sh[0] = lo[0]; sh[1] = lo[1]; sh[2] = lo[2];
-            sh[3] = (ext > 0.f && ext < 3.0e38f) ? kCells / ext : 0.f;
-        }
-    }
-    __syncthreads();
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n) return;
-    const float4 p = posm[i];
-    const float sc = sh[3];
-    const uint32_t qx = (uint32_t)fminf(fmaxf((p.x - sh[0]) * sc, 0.f), kCells);
-    const uint32_t qy = (uint32_t)fminf(fmaxf((p.y - sh[1]) * sc, 0.f), kCells);
-    const uint32_t qz = (uint32_t)fminf(fmaxf((p.z - sh[2]) * sc, 0.f), kCells);
-    keys[i] = hilbert_key(qx, qy, qz, bits);
-    vals[i] = (uint32_t)i;
 }
 
 // One 1024-thread block per super-group.  gbox[2g] = (lo.xyz, Rmax), gbox[2g+1] = (hi.xyz, 0);
@@ -646,16 +549,14 @@ nb_gather_kernel(const float4* __restrict__ posm, const float4* __restrict__ vel
 }
 
 struct ContactArgs {
-    const float4* __restrict__ ps;     // [n] x,y,z,R_star   (Hilbert order)
+    const float4* __restrict__ ps;     // [n] x,y,z,R_star
     const float4* __restrict__ vs;     // [n] vx,vy,vz,m
     const uint32_t* __restrict__ perm; // [n] original index of sorted element k (nullptr: identity)
     const float4* __restrict__ gbox;   // [2*ngroups]
     const float4* __restrict__ sbox;   // [2*nsuper]
     float4* __restrict__ out;          // [nchunks][n] contact acceleration, ORIGINAL index order
     int n, ngroups, nsuper;
-    int nchunks;                       // nb_contact_kernel: the candidate groups of a group of elements i are dealt
-                                       // round-robin to nchunks warps (neighbours are adjacent on the Hilbert curve, so
-                                       // a split by ranges would leave all the work with one warp)
+    int nchunks;                       // slabs of `out` (index-order search: one per chunk of candidate groups)
     float gamma, gamma_beta;           // Eq. 5 / Eq. 6 strengths
     float v_dead;
     int lens_mode;
@@ -775,73 +676,6 @@ __device__ __forceinline__ void contact_candidates(const ContactArgs& a, const i
             if (r1 <= t1 && valid) { hq[nh * 32 + lane] = (uint32_t)(j0 + t + 1); ++nh; }
         }
         if (__any_sync(0xffffffffu, nh >= kHitFlush)) contact_drain(a, hq, nh, pi, vi, lane, ax, ay, az);
-    }
-}
-
-__global__ void __launch_bounds__(kThreads)
-nb_contact_kernel(const __grid_constant__ ContactArgs a)
-{
-    __shared__ int cand_s[kThreads / 32][kCandCap];
-    __shared__ float4 stage_s[kThreads / 32][kGroup];
-    __shared__ uint32_t hit_s[kThreads / 32][kHitCap * 32];
-    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    uint32_t* hq = hit_s[wib];
-    int nh = 0;
-    const int wid = (blockIdx.x * kThreads + threadIdx.x) >> 5;
-    const int ig = wid / a.nchunks, ch = wid - ig * a.nchunks;     // group of elements i, chunk of super-groups
-    if (ig >= a.ngroups) return;
-    const int sb0 = 0, sb1 = a.nsuper;             // every chunk warp scans all boxes; the candidates are dealt round-robin
-    int tot = 0;                                    // candidate groups found so far (the same in every chunk warp)
-    int* cand = cand_s[wib];
-    float4* stage = stage_s[wib];
-    const int k = ig * kGroup + lane;
-    const bool valid = k < a.n;
-    const float4 pi = valid ? a.ps[k] : make_float4(kFarAway, kFarAway, kFarAway, 0.f);
-    const float4 vi = valid ? a.vs[k] : make_float4(0.f, 0.f, 0.f, 1.f);
-    const float4 ilo = a.gbox[2 * ig], ihi = a.gbox[2 * ig + 1];
-    const float kSlack = 1.0f + 1.0e-5f;                            // the box and fp32 pair tests are pre-filters
-    double ax = 0.0, ay = 0.0, az = 0.0;
-    int cnt = 0;
-
-    for (int sb = sb0; sb < sb1; sb += 32) {
-        bool near = false;
-        if (sb + lane < sb1) {
-            const float4 lo = a.sbox[2 * (sb + lane)], hi = a.sbox[2 * (sb + lane) + 1];
-            const float D = ilo.w + lo.w;
-            near = box_gap2(ilo, ihi, lo, hi) <= D * D * kSlack;
-        }
-        unsigned smask = __ballot_sync(0xffffffffu, near);
-        while (smask) {
-            const int s = sb + __ffs(smask) - 1;
-            smask &= smask - 1;
-            const int g = s * kSuper + lane;
-            bool gnear = false;
-            if (g < a.ngroups) {
-                const float4 lo = a.gbox[2 * g], hi = a.gbox[2 * g + 1];
-                const float D = ilo.w + lo.w;
-                gnear = box_gap2(ilo, ihi, lo, hi) <= D * D * kSlack;
-            }
-            const unsigned fmask = __ballot_sync(0xffffffffu, gnear);
-            gnear = gnear && ((tot + __popc(fmask & ((1u << lane) - 1u))) % a.nchunks == ch);
-            tot += __popc(fmask);
-            const unsigned gmask = __ballot_sync(0xffffffffu, gnear);
-            const int m = __popc(gmask);
-            if (cnt + m > kCandCap) {                               // flush the list before it overflows
-                __syncwarp();
-                contact_candidates(a, cand, cnt, stage, hq, nh, pi, vi, valid, lane, ax, ay, az);
-                cnt = 0;
-                __syncwarp();
-            }
-            if (gnear) cand[cnt + __popc(gmask & ((1u << lane) - 1u))] = g;
-            cnt += m;
-        }
-    }
-    __syncwarp();
-    contact_candidates(a, cand, cnt, stage, hq, nh, pi, vi, valid, lane, ax, ay, az);
-    contact_drain(a, hq, nh, pi, vi, lane, ax, ay, az);
-    if (valid) {
-        const int dst = a.perm ? (int)a.perm[k] : k;
-        a.out[(size_t)ch * a.n + dst] = make_float4((float)ax, (float)ay, (float)az, 0.f);
     }
 }
 
