@@ -36,6 +36,8 @@ constexpr int64_t kMaxSplit = 64;
 constexpr int64_t kPartialBudget = (int64_t)128 << 20;   // bytes of split-j partial sums worth keeping in L2
 constexpr int64_t kCellMinN = 8192;                // below this the contact pass takes groups in index order (all pairs
                                                    // pre-tested), from here on it builds the cell list
+constexpr int64_t kContactWideN = 131072;          // cell list: below this, 4 lanes share the rows of an element's query
+                                                   // (measured: 16,384: 45 vs 67 us per pass, 65,536: 50 vs 53; 262,144: 129 vs 107)
 constexpr int kMaxContactChunks = 32;              // index-order search: the candidate groups of a warp go to this many slabs
 
 // Force-path selection (nb_set_force_path).
@@ -159,7 +161,7 @@ Layout make_layout(int64_t n_max)
     L.off_gbox = o; o += align_up(ngroups * 2 * sizeof(float4));
     L.off_sbox = o; o += align_up(nsuper * 2 * sizeof(float4));
     const size_t ncnt = (size_t)cell_counters_bound(n_max);
-    L.off_cpart = o;    o += align_up((size_t)kBoxBlocks * 2 * sizeof(CellPartial));
+    L.off_cpart = o;    o += align_up((size_t)kPassMaxBlocks * 2 * sizeof(CellPartial));
     L.off_cstate = o;   o += align_up(sizeof(CellState));
     L.off_counters = o; o += align_up(ncnt * sizeof(int));
     L.off_bsum = o;     o += align_up((ncnt / kCellScanChunk + 2) * sizeof(int));
@@ -275,6 +277,20 @@ int launch_gravity(nb_ctx* c)
     return NB_OK;
 }
 
+// Launch `kernel` behind the previous kernel of the stream; with `pdl` as its programmatic dependent (the kernel
+// starts launching before its predecessor has finished and waits for it in pdl_prologue()).
+template <class... P, class... A>
+cudaError_t launch_after(bool pdl, void (*kernel)(P...), int grid, int block, cudaStream_t st, A... args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = pdl ? 1 : 0;
+    return cudaLaunchKernelEx(&cfg, kernel, P(args)...);
+}
+
 // Row a3: contact accelerations (Eqs. 5/6) of the pairs with r < R_i + R_j -> part[ngrav ...][n]
 int launch_contact_on(nb_ctx* c, cudaStream_t st)
 {
@@ -287,28 +303,35 @@ int launch_contact_on(nb_ctx* c, cudaStream_t st)
     ca.v_dead = c->prm.v_dead; ca.lens_mode = c->prm.lens_mode;
     if (c->n >= kCellMinN) {                                      // cell list (nb_cells.cuh)
         const Layout& L = c->lay;
-        CellArgs a;
+        CellPassArgs a;
         a.posm = c->posm; a.vel = c->vel; a.dev = c->dev();
         a.part = c->at<CellPartial>(L.off_cpart); a.cs = c->at<CellState>(L.off_cstate);
         a.counters = c->at<int>(L.off_counters); a.bsum = c->at<int>(L.off_bsum);
         a.bucket = c->at<int>(L.off_bucket); a.slot = c->at<int>(L.off_slot); a.tmp = c->at<int>(L.off_tmp);
         a.perm = c->at<uint32_t>(L.off_perm); a.ps = c->ps(); a.vs = c->vs();
+        a.out = ca.out; a.law = ca;
         a.n = n; a.n1 = c->n1;
         a.cap0 = (int)cell_cap(c->n1); a.cap1 = (int)cell_cap(c->n - c->n1); a.ncells = a.cap0 + a.cap1;
-        const int eb = (n + 255) / 256;
+        a.lpe_log2 = c->n < kContactWideN ? 2 : 0;                  // lanes per element: 4 while the pass is latency-bound
+        const long long eb = (n + kPassThreads - 1) / kPassThreads;
+        long long cb;
+        a.nparts = (int)(eb < kBoxBlocks ? eb : kBoxBlocks);
         const int sb = (a.ncells + kCellScanChunk - 1) / kCellScanChunk;
-        nb_cell_bbox_kernel<<<kBoxBlocks, 256, 0, st>>>(c->posm, n, c->n1, c->at<CellPartial>(L.off_cpart), a.counters,
-                                                       a.ncells + 1);
-        nb_cell_count_kernel<<<eb, 256, 0, st>>>(a);
-        if (sb > 1) { nb_cell_scan_kernel<<<sb, 1024, 0, st>>>(a.counters, a.bsum, a.ncells, 0); c->launches++; }
-        nb_cell_scan_kernel<<<sb, 1024, 0, st>>>(a.counters, a.bsum, a.ncells, 1);
-        nb_cell_scatter_kernel<<<eb, 256, 0, st>>>(a);
-        nb_cell_rank_kernel<<<eb, 256, 0, st>>>(a);
-        CellContactArgs k;
-        k.ps = c->ps(); k.vs = c->vs(); k.perm = a.perm; k.start = a.counters; k.cs = a.cs; k.dev = c->dev();
-        k.out = ca.out; k.law = ca; k.n = n;
-        nb_contact_cell_kernel<<<(n + kThreads - 1) / kThreads, kThreads, 0, st>>>(k);
-        c->launches += 6;
+        const bool pdl = true;
+        nb_cell_bbox_kernel<<<a.nparts, kPassThreads, 0, st>>>(a);
+        NB_CUDA(c, launch_after(pdl, nb_cell_count_kernel, (int)eb, kPassThreads, st, a));
+        NB_CUDA(c, launch_after(pdl, nb_cell_scan_kernel, sb, kPassThreads, st, a, 0));
+        NB_CUDA(c, launch_after(pdl, nb_cell_scan_kernel, sb, kPassThreads, st, a, 3));
+        NB_CUDA(c, launch_after(pdl, nb_cell_scatter_kernel, (int)eb, kPassThreads, st, a));
+        NB_CUDA(c, launch_after(pdl, nb_cell_rank_kernel, (int)eb, kPassThreads, st, a));
+        cb = (((long long)n << a.lpe_log2) + kCcThreads - 1) / kCcThreads;
+        switch (a.lpe_log2) {
+            case 0: NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<0>, (int)cb, kCcThreads, st, a)); break;
+            case 1: NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<1>, (int)cb, kCcThreads, st, a)); break;
+            case 2: NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<2>, (int)cb, kCcThreads, st, a)); break;
+            default: NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<3>, (int)cb, kCcThreads, st, a)); break;
+        }
+        c->launches += 7;
         NB_CUDA(c, cudaGetLastError());
         return NB_OK;
     }

@@ -3,10 +3,9 @@
 // Hot path:
 //   a2     nb_gravity_sym_kernel    all-pairs Eq. 4 gravity, every unordered pair once
 //          nb_gravity_kernel        the same sum over every ordered pair (small and very large n)
-//   a3     nb_contact_kernel        contact terms of Eqs. 5/6 for exactly the
-//                                   pairs with r < R_i + R_j, found through Hilbert-ordered groups
-//                                   of 32 elements and their bounding boxes
-//          (nb_bbox_kernel, nb_keys_kernel, [radix sort], nb_gather_kernel build that order)
+//   a3     nb_contact_cell_kernel   contact terms of Eqs. 5/6 for exactly the
+//                                   pairs with r < R_i + R_j, found through a cell list (nb_cells.cuh);
+//          nb_contact_chunk_kernel  the same for n < 8,192, every pair pre-tested
 //   a4/a6  nb_reduce_update_kernel  partial-sum reduction fused with the leapfrog kick/drift and
 //                                   the expanding-star rule
 //   a7     nb_potential_kernel / nb_moments_kernel   diagnostics for nb_energy
