@@ -168,7 +168,7 @@ int nb_download_state(nb_ctx* ctx, float* host_posm, float* host_vel, float* hos
 int nb_get_launch_info(nb_ctx* ctx, int32_t* out4);
 
 /* Which kernel evaluates row a2 (Eq. 4, summed over all pairs).
- *   NB_PATH_AUTO (default): the symmetric kernel for 24576 <= n <= 2097152, else the one-sided
+ *   NB_PATH_AUTO (default): the symmetric kernel for 10240 <= n <= 2097152, else the one-sided
  *     kernel (the symmetric kernel is never used above 2097152 elements: its partial sums would
  *     not fit; NB_PATH_SYMMETRIC then falls back to the one-sided kernel as well).
  *   NB_PATH_ONE_SIDED: every ORDERED pair (i, j) is evaluated; a CTA owns an (i-block, j-split).

@@ -14,7 +14,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libnb.so")
 SOURCES = [os.path.join(CSRC, "nb_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "nb_kernels.cuh"), os.path.join(CSRC, "nb_cells.cuh"),
+DEPS = SOURCES + [os.path.join(CSRC, "nb_kernels.cuh"), os.path.join(CSRC, "nb_cells.cuh"), os.path.join(CSRC, "nb_fused.cuh"),
                   os.path.join(ROOT, "include", "nb.h")]
 
 NVCC_FLAGS = [

@@ -4,6 +4,7 @@
 #include "nb.h"
 #include "nb_kernels.cuh"
 #include "nb_cells.cuh"
+#include "nb_fused.cuh"
 
 #include <cmath>
 #include <cstdio>
@@ -42,9 +43,10 @@ constexpr int kMaxContactChunks = 32;              // index-order search: the ca
 
 // Force-path selection (nb_set_force_path).
 enum { kPathAuto = 0, kPathOneSided = 1, kPathSymmetric = 2 };
-constexpr int64_t kSymMinN = 24576;               // auto: symmetric kernel from here on.  The kernel alone wins from ~6,000
+constexpr int64_t kSymMinN = 10240;               // auto: symmetric kernel from here on.  The kernel alone wins from ~6,000
                                                   // elements, but its 126 registers leave the contact pass no room to run
-                                                  // beside it: whole steps are equal at 16,384 and 10 % shorter at 24,576
+                                                  // beside it; measured whole steps (one-sided / symmetric, us): 8,192: 64 / 67,
+                                                  // 10,240: 79 / 78, 12,288: 105 / 89, 16,384: 164 / 137, 24,576: 331 / 243
 constexpr int64_t kSym256MaxN = 32768;             // below this the super-tiles are 256 elements (CTAs of 2 warps)
 constexpr int64_t kSymMaxN = (int64_t)1 << 21;    // ... up to here: its T slabs of n float4 reach 17 GB at 2M elements
 
@@ -125,6 +127,7 @@ Plan make_plan(int64_t n, int num_sms, int path)
     p.njt = (int)((n + p.TJ - 1) / p.TJ);
     const int64_t slots = (int64_t)num_sms * kCtasPerSM;
     int64_t pmax = p.njt >= 2 ? p.njt / 2 : 1;
+    if (n < kCellMinN) pmax = p.njt;                 // small n (one fused launch, see nb_fused.cuh): down to one tile per CTA
     if (pmax > max_split(n)) pmax = max_split(n);
     double best = 0.0;
     for (int64_t P = 1; P <= pmax; ++P) {
@@ -183,6 +186,7 @@ struct nb_ctx {
     cudaStream_t side = nullptr;          // library-owned: the contact pass runs here, beside the gravity kernel
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int num_sms = kNumSMsFallback;
+    int fused_blocks = 0;                 // co-resident CTAs of nb_fused_step_kernel (cooperative launch); 0: not available
     float4* posm = nullptr;
     float4* vel = nullptr;
     char* ws = nullptr;
@@ -386,9 +390,41 @@ int launch_update(nb_ctx* c, const float4* src, int nsrc, float4* acc_out, float
     return NB_OK;
 }
 
+// n < kCellMinN: rows a2-a6 for `nforce` force evaluations in ONE cooperative launch (nb_fused.cuh).
+bool fused_path(const nb_ctx* c) { return c->n < kCellMinN && !c->plan.sym_S && c->fused_blocks > 0; }
+
+int launch_fused(nb_ctx* c, int nforce, int open, int close_mode, float4* acc_out)
+{
+    FusedArgs f;
+    std::memset(&f, 0, sizeof(f));
+    const int n = (int)c->n;
+    f.grav.posm = c->posm; f.grav.part = c->part();
+    f.grav.n = n; f.grav.nib = c->plan.nib; f.grav.nsplit = c->plan.nsplit; f.grav.njt = c->plan.njt;
+    f.grav.G = c->prm.G; f.grav.eps = c->prm.eps;
+    f.law.n = n;
+    f.law.gamma = c->prm.gamma; f.law.gamma_beta = c->prm.gamma * c->prm.beta;
+    f.law.v_dead = c->prm.v_dead; f.law.lens_mode = c->prm.lens_mode;
+    f.posm = c->posm; f.vel = c->vel; f.acc = c->acc(); f.acc_out = acc_out;
+    f.dev = c->dev(); f.n = n; f.n1 = c->n1; f.dt = c->prm.dt;
+    f.nforce = nforce; f.open = open; f.close_mode = close_mode;
+    long long blocks = (long long)c->plan.nib * c->plan.nsplit;      // one CTA per work item if they fit
+    if (blocks > c->fused_blocks) blocks = c->fused_blocks;
+    void* args[] = {&f};
+    NB_CUDA(c, cudaLaunchCooperativeKernel((const void*)nb_fused_step_kernel, dim3((unsigned)blocks), dim3(kThreads), args, 0,
+                                           c->stream));
+    c->launches++;
+    return NB_OK;
+}
+
 int ensure_acc(nb_ctx* c)
 {
     if (c->have_acc) return NB_OK;
+    if (fused_path(c)) {
+        const int rc = launch_fused(c, 1, 0, 1, nullptr);
+        if (rc) return rc;
+        c->have_acc = true;
+        return NB_OK;
+    }
     int rc = launch_force(c);
     if (rc) return rc;
     rc = launch_update(c, c->part(), c->nslabs(), c->acc(), 0.f, 0.f, 0);
@@ -446,6 +482,12 @@ int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream
         cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
         nb_destroy(c);
         return NB_ECUDA;
+    }
+    {   // CTAs of the fused small-n kernel that can be resident together (it synchronises grid-wide between its phases)
+        int per_sm = 0, coop = 0;
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
+        if (coop && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, nb_fused_step_kernel, kThreads, 0) == cudaSuccess)
+            c->fused_blocks = per_sm * c->num_sms;
     }
     // the symmetric kernel's shared memory is dynamic (112 KB at S = 4096)
     if (cudaFuncSetAttribute(NB_SYM_512, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 512) != cudaSuccess ||
@@ -511,6 +553,12 @@ int nb_compute_accel(nb_ctx* c, float* acc)
 {
     if (!c || !acc || ((uintptr_t)acc & 15)) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (fused_path(c)) {
+        const int rc = launch_fused(c, 1, 0, 1, reinterpret_cast<float4*>(acc) != c->acc() ? reinterpret_cast<float4*>(acc) : nullptr);
+        if (rc) return rc;
+        c->have_acc = true;
+        return NB_OK;
+    }
     int rc = launch_force(c);
     if (rc) return rc;
     rc = launch_update(c, c->part(), c->nslabs(), reinterpret_cast<float4*>(acc), 0.f, 0.f, 0);
@@ -531,6 +579,7 @@ int nb_step(nb_ctx* c, int nsteps)
     const float dt = c->prm.dt;
     int rc = ensure_acc(c);                                    // a(x_n) with v_n (A7)
     if (rc) return rc;
+    if (fused_path(c)) return launch_fused(c, nsteps, 1, 0, nullptr);   // all nsteps in one launch
     // v_{n+1/2} = v_n + dt/2 a_n ; x_{n+1} = x_n + dt v_{n+1/2} ; n += 1, R(n)
     rc = launch_update(c, c->acc(), 1, nullptr, 0.5f * dt, dt, 1);
     if (rc) return rc;

@@ -311,43 +311,6 @@ __device__ __forceinline__ void cell_phase_rank(const CellPassArgs& a)
     }
 }
 
-// One contact pair, Eqs. 5/6, as the acceleration it gives element i (x m_i: the caller
-// multiplies by 1/m_i).  Same decisions and the same exact fp64 differences as contact_term(); 1/r comes from
-// the fp32 MUFU.RSQ seed refined by two Newton steps in fp64 (relative error ~2^-52) instead of a
-// double-precision square root and division (~10 instead of ~60 fp64-pipe instructions).
-__device__ __forceinline__ void contact_pair(const ContactArgs& a, const float4 pi, const float4 vi, const float4 pj,
-                                             const float4 vj, double& fx, double& fy, double& fz)
-{
-    fx = fy = fz = 0.0;
-    const double dx = (double)pj.x - (double)pi.x, dy = (double)pj.y - (double)pi.y, dz = (double)pj.z - (double)pi.z;
-    const double r2 = dx * dx + dy * dy + dz * dz;
-    const double D = (double)pi.w + (double)pj.w;                   // R_i + R_j = 2 R_ij (A2)
-    if (!(r2 < D * D) || r2 == 0.0) return;                         // not in contact / coincident (A3)
-    double y;
-    if (r2 > 1.0e-30) {
-        y = (double)rsqrt_approx((float)r2);
-        y = y * (1.5 - 0.5 * r2 * y * y);
-        y = y * (1.5 - 0.5 * r2 * y * y);
-    } else {
-        y = 1.0 / sqrt(r2);
-    }
-    const double r = r2 * y;
-    const double rdot = (dx * ((double)vj.x - (double)vi.x) + dy * ((double)vj.y - (double)vi.y)
-                       + dz * ((double)vj.z - (double)vi.z)) * y;
-    const double g = (rdot < -(double)a.v_dead) ? (double)a.gamma : (double)a.gamma_beta;  // Eq. 5 : Eq. 6 (A5)
-    const double kPi = 3.14159265358979323846;
-    double piV;
-    if (a.lens_mode == 0) {
-        const double h = D - r;
-        piV = (kPi / 12.0) * h * h * (2.0 * D + r);
-    } else {
-        const double R = 0.5 * D;
-        piV = kPi * ((4.0 / 3.0) * R * R * R - R * R * r + r * r / 12.0);
-    }
-    const double c = -g * piV * y;
-    fx = c * dx; fy = c * dy; fz = c * dz;
-}
-
 constexpr int kCcThreads = 128;        // threads per block of the contact kernel
 constexpr int kCcQueue = 16;           // per-lane queue of pairs that passed the fp32 pre-test
 constexpr int kCcRound = 64;           // pairs a warp evaluates per round of the balanced evaluation

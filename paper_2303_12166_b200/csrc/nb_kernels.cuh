@@ -93,19 +93,36 @@ __device__ __forceinline__ float star_radius(int idx, int n1, float R0, float R1
 // elements) skip the per-pair multiply by G m_j: the tile's fp32 sums are
 // scaled once when they are flushed into the fp64 accumulators.  Other tiles multiply k by
 // G m_j (one more FMUL2 per lane pair and j).
+// (No __restrict__ on these members: nb_fused_step_kernel writes the same arrays in another phase of the same
+// launch, and loads through the read-only path would then be undefined.)
 struct GravArgs {
-    const float4* __restrict__ posm;   // [n] x,y,z,m
-    float4* __restrict__ part;         // [nsplit][n] partial accelerations
+    const float4* posm;                // [n] x,y,z,m
+    float4* part;                      // [nsplit][n] partial accelerations
     int n, nib, nsplit, njt;
     float G, eps;
 };
 
 constexpr int kGroupJ = 4;             // elements j per unrolled group (two Montgomery pairs)
 
-template <int H, bool UNI>
+// Contact terms found INSIDE the all-pairs loop (CON = true: the fused small-n kernel, where a separate contact
+// pass would be one more chain of latencies; the big kernels keep the test out of the loop, see 5.1b of DESIGN.md).
+struct ContactArgs;
+__device__ __forceinline__ void contact_pair(const ContactArgs& a, const float4 pi, const float4 vi, const float4 pj,
+                                             const float4 vj, double& fx, double& fy, double& fz);
+constexpr int kInlineQueue = 24;       // per-thread queue of (i slot, j) pairs that passed the fp32 pre-test
+struct InlineContact {
+    const ContactArgs* law;            // gamma, gamma_beta, v_dead, lens_mode
+    const float4* vel;                 // [n]
+    int n1;
+    float R0, R1;                      // element radius per star
+    uint32_t* q;                       // the thread's queue: q[k * kThreads], k < kInlineQueue
+};
+
+template <int H, bool UNI, bool CON>
 __device__ __forceinline__ void gravity_group(const float4* __restrict__ s,
                                               const f32x2 (&nxi)[H], const f32x2 (&nyi)[H], const f32x2 (&nzi)[H],
-                                              f32x2 eps2, f32x2 (&ax)[H], f32x2 (&ay)[H], f32x2 (&az)[H])
+                                              f32x2 eps2, f32x2 (&ax)[H], f32x2 (&ay)[H], f32x2 (&az)[H],
+                                              const float thr, const int jglob, uint32_t* __restrict__ q, int& nq)
 {
     const f32x2 tiny2 = pk2(kTinyR2, kTinyR2);
 #pragma unroll
@@ -121,6 +138,15 @@ __device__ __forceinline__ void gravity_group(const float4* __restrict__ s,
             f32x2 r21 = fma2(dx1, dx1, tiny2); r21 = fma2(dy1, dy1, r21); r21 = fma2(dz1, dz1, r21);
             float a0, b0, a1, b1;
             unpk2(r20, a0, b0); unpk2(r21, a1, b1);
+            if (CON) {                               // within reach of a contact (or the self pair): queue for the fp64 test
+                if (fminf(fminf(a0, b0), fminf(a1, b1)) <= thr) {
+                    const uint32_t j0 = (uint32_t)(jglob + u), sl = (uint32_t)(2 * h);
+                    if (a0 <= thr) q[(nq++) * kThreads] = (j0 << 4) | sl;
+                    if (b0 <= thr) q[(nq++) * kThreads] = (j0 << 4) | (sl + 1);
+                    if (a1 <= thr) q[(nq++) * kThreads] = ((j0 + 1) << 4) | sl;
+                    if (b1 <= thr) q[(nq++) * kThreads] = ((j0 + 1) << 4) | (sl + 1);
+                }
+            }
             const f32x2 ri0 = pk2(rsqrt_approx(a0), rsqrt_approx(b0));     // 1/r
             const f32x2 ri1 = pk2(rsqrt_approx(a1), rsqrt_approx(b1));
             const f32x2 s0 = fma2(r20, ri0, eps2), s1 = fma2(r21, ri1, eps2);   // r + eps
@@ -138,18 +164,19 @@ __device__ __forceinline__ void gravity_group(const float4* __restrict__ s,
     }
 }
 
-template <int I, int TJ>
-__global__ void __launch_bounds__(kThreads, (I == 2 ? 8 : 4))
-nb_gravity_kernel(const __grid_constant__ GravArgs a)
+// The work of one CTA (i-block, j-split) = block `vb` of a grid of nib * nsplit; sj: the CTA's two tiles.
+template <int I, int TJ, bool CON = false>
+__device__ __forceinline__ void gravity_block(const GravArgs& a, const int vb, float4 (*sj)[TJ],
+                                              const InlineContact ic = InlineContact())
 {
     static_assert(I % 2 == 0 && TJ % kThreads == 0 && TJ % kGroupJ == 0, "packed pairs; whole groups");
+    static_assert(I <= 16 && kInlineQueue >= 2 * kGroupJ * I, "queue entries carry the i slot in 4 bits; a group adds <= 4 I");
     constexpr int H = I / 2;                        // packed pairs per thread
     constexpr int LPT = TJ / kThreads;              // tile loads per thread
-    __shared__ float4 sj[2][TJ];
 
     const int tid = threadIdx.x;
-    const int ib = blockIdx.x % a.nib;
-    const int sp = blockIdx.x / a.nib;
+    const int ib = vb % a.nib;
+    const int sp = vb / a.nib;
     const int ibase = ib * (kThreads * I) + tid;    // element k of this thread: ibase + k*kThreads
 
     f32x2 nxi[H], nyi[H], nzi[H];                   // (-x_i) of the two lanes
@@ -175,6 +202,60 @@ nb_gravity_kernel(const __grid_constant__ GravArgs a)
     double accx[I], accy[I], accz[I];
 #pragma unroll
     for (int k = 0; k < I; ++k) accx[k] = accy[k] = accz[k] = 0.0;
+
+    // inline contact search: one fp32 threshold per thread and tile, (largest R_i of the thread's elements +
+    // largest R_j of the tile)^2 -- tiles rarely straddle the two stars, so this is the pair's own reach
+    float thr = -1.f, Rm = 0.f;
+    int nq = 0;
+    uint32_t* __restrict__ q = ic.q;
+    if (CON) {
+#pragma unroll
+        for (int k = 0; k < I; ++k) Rm = fmaxf(Rm, star_radius(min(ibase + k * kThreads, a.n - 1), ic.n1, ic.R0, ic.R1));
+    }
+    // what contact_pair() needs of the thread's own elements: (x, R) and (v, m); x_j comes from the tile in shared
+    // memory, so a queued pair costs ONE global load (v_j)
+    float4 cpi[CON ? I : 1], cvi[CON ? I : 1];
+    if (CON) {
+#pragma unroll
+        for (int k = 0; k < I; ++k) {
+            const int i = min(ibase + k * kThreads, a.n - 1);
+            const float4 x = a.posm[i], w = ic.vel[i];
+            cpi[k] = make_float4(x.x, x.y, x.z, star_radius(i, ic.n1, ic.R0, ic.R1));
+            cvi[k] = make_float4(w.x, w.y, w.z, x.w);
+        }
+    }
+    const float4* tile = nullptr;                    // the tile being walked, and the index of its first element
+    int tile_j0 = 0;
+    auto drain = [&]() {                             // the queued pairs, in the order found, in fp64
+        for (int e0 = 0; e0 < nq; e0 += 2) {
+            int jj[2], kk[2];
+            float4 wj[2];
+            bool ok[2];
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {            // both loads in flight together
+                const uint32_t w = q[min(e0 + u, nq - 1) * kThreads];
+                jj[u] = (int)(w >> 4); kk[u] = (int)(w & 15u);
+                ok[u] = e0 + u < nq && jj[u] < a.n && ibase + kk[u] * kThreads < a.n && jj[u] != ibase + kk[u] * kThreads;
+                wj[u] = ok[u] ? ic.vel[jj[u]] : make_float4(0.f, 0.f, 0.f, 0.f);
+            }
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                if (!ok[u]) continue;
+                const float4 xj = tile[jj[u] - tile_j0];
+                float4 pi = cpi[0], vi = cvi[0];
+#pragma unroll
+                for (int k = 1; k < I; ++k) if (k == kk[u]) { pi = cpi[k]; vi = cvi[k]; }
+                double fx, fy, fz;
+                contact_pair(*ic.law, pi, vi, make_float4(xj.x, xj.y, xj.z, star_radius(jj[u], ic.n1, ic.R0, ic.R1)), wj[u],
+                             fx, fy, fz);
+                const double im = 1.0 / (double)vi.w;
+#pragma unroll
+                for (int k = 0; k < I; ++k)
+                    if (k == kk[u]) { accx[k] += fx * im; accy[k] += fy * im; accz[k] += fz * im; }
+            }
+        }
+        nq = 0;
+    };
 
     float4 pre[LPT];
     bool my_uni = false;                             // this thread's share of the tile has one mass
@@ -214,17 +295,28 @@ nb_gravity_kernel(const __grid_constant__ GravArgs a)
         for (int h = 0; h < H; ++h) ax[h] = ay[h] = az[h] = pk2(0.f, 0.f);
 
         const float4* __restrict__ s = sj[buf];
+        tile = s; tile_j0 = t * TJ;
+        if (CON) {
+            const float Rj = (t + 1) * TJ <= ic.n1 ? ic.R0 : (t * TJ >= ic.n1 ? ic.R1 : fmaxf(ic.R0, ic.R1));
+            const float D = Rm + Rj;
+            thr = D * D * (1.0f + 1.0e-5f) + kTinyR2;
+        }
         double scale = 1.0;
         if (uni) {
 #pragma unroll 1
-            for (int jg = 0; jg < TJ; jg += kGroupJ)
-                gravity_group<H, true>(s + jg, nxi, nyi, nzi, eps2, ax, ay, az);
+            for (int jg = 0; jg < TJ; jg += kGroupJ) {
+                gravity_group<H, true, CON>(s + jg, nxi, nyi, nzi, eps2, ax, ay, az, thr, t * TJ + jg, q, nq);
+                if (CON && nq > kInlineQueue - 2 * kGroupJ * H) drain();
+            }
             scale = (double)s[0].w;                  // G m of the whole tile
         } else {
 #pragma unroll 1
-            for (int jg = 0; jg < TJ; jg += kGroupJ)
-                gravity_group<H, false>(s + jg, nxi, nyi, nzi, eps2, ax, ay, az);
+            for (int jg = 0; jg < TJ; jg += kGroupJ) {
+                gravity_group<H, false, CON>(s + jg, nxi, nyi, nzi, eps2, ax, ay, az, thr, t * TJ + jg, q, nq);
+                if (CON && nq > kInlineQueue - 2 * kGroupJ * H) drain();
+            }
         }
+        if (CON) drain();
 
         // flush the tile's fp32 sums into the fp64 accumulators (short fp32 chains)
 #pragma unroll
@@ -245,6 +337,14 @@ nb_gravity_kernel(const __grid_constant__ GravArgs a)
         const int i = ibase + k * kThreads;
         if (i < a.n) out[i] = make_float4((float)accx[k], (float)accy[k], (float)accz[k], 0.f);
     }
+}
+
+template <int I, int TJ>
+__global__ void __launch_bounds__(kThreads, (I == 2 ? 8 : 4))
+nb_gravity_kernel(const __grid_constant__ GravArgs a)
+{
+    __shared__ float4 sj[2][TJ];
+    gravity_block<I, TJ>(a, blockIdx.x, sj);
 }
 
 // ---------------------------------------------------------------------------
@@ -548,12 +648,12 @@ nb_gather_kernel(const float4* __restrict__ posm, const float4* __restrict__ vel
 }
 
 struct ContactArgs {
-    const float4* __restrict__ ps;     // [n] x,y,z,R_star
-    const float4* __restrict__ vs;     // [n] vx,vy,vz,m
-    const uint32_t* __restrict__ perm; // [n] original index of sorted element k (nullptr: identity)
-    const float4* __restrict__ gbox;   // [2*ngroups]
-    const float4* __restrict__ sbox;   // [2*nsuper]
-    float4* __restrict__ out;          // [nchunks][n] contact acceleration, ORIGINAL index order
+    const float4* ps;                  // [n] x,y,z,R_star
+    const float4* vs;                  // [n] vx,vy,vz,m
+    const uint32_t* perm;              // [n] original index of sorted element k (nullptr: identity)
+    const float4* gbox;                // [2*ngroups]
+    const float4* sbox;                // [2*nsuper]
+    float4* out;                       // [nchunks][n] contact acceleration, ORIGINAL index order
     int n, ngroups, nsuper;
     int nchunks;                       // slabs of `out` (index-order search: one per chunk of candidate groups)
     float gamma, gamma_beta;           // Eq. 5 / Eq. 6 strengths
@@ -599,6 +699,43 @@ __device__ __forceinline__ void contact_term(const ContactArgs& a, const float4 
     }
     const double c = -g * piV / (double)vi.w * rinv;                // vi.w = m_i
     ax += c * dx; ay += c * dy; az += c * dz;
+}
+
+// One contact pair, Eqs. 5/6, as the acceleration it gives element i (x m_i: the caller
+// multiplies by 1/m_i).  Same decisions and the same exact fp64 differences as contact_term(); 1/r comes from
+// the fp32 MUFU.RSQ seed refined by two Newton steps in fp64 (relative error ~2^-52) instead of a
+// double-precision square root and division (~10 instead of ~60 fp64-pipe instructions).
+__device__ __forceinline__ void contact_pair(const ContactArgs& a, const float4 pi, const float4 vi, const float4 pj,
+                                             const float4 vj, double& fx, double& fy, double& fz)
+{
+    fx = fy = fz = 0.0;
+    const double dx = (double)pj.x - (double)pi.x, dy = (double)pj.y - (double)pi.y, dz = (double)pj.z - (double)pi.z;
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double D = (double)pi.w + (double)pj.w;                   // R_i + R_j = 2 R_ij (A2)
+    if (!(r2 < D * D) || r2 == 0.0) return;                         // not in contact / coincident (A3)
+    double y;
+    if (r2 > 1.0e-30) {
+        y = (double)rsqrt_approx((float)r2);
+        y = y * (1.5 - 0.5 * r2 * y * y);
+        y = y * (1.5 - 0.5 * r2 * y * y);
+    } else {
+        y = 1.0 / sqrt(r2);
+    }
+    const double r = r2 * y;
+    const double rdot = (dx * ((double)vj.x - (double)vi.x) + dy * ((double)vj.y - (double)vi.y)
+                       + dz * ((double)vj.z - (double)vi.z)) * y;
+    const double g = (rdot < -(double)a.v_dead) ? (double)a.gamma : (double)a.gamma_beta;  // Eq. 5 : Eq. 6 (A5)
+    const double kPi = 3.14159265358979323846;
+    double piV;
+    if (a.lens_mode == 0) {
+        const double h = D - r;
+        piV = (kPi / 12.0) * h * h * (2.0 * D + r);
+    } else {
+        const double R = 0.5 * D;
+        piV = kPi * ((4.0 / 3.0) * R * R * R - R * R * r + r * r / 12.0);
+    }
+    const double c = -g * piV * y;
+    fx = c * dx; fy = c * dy; fz = c * dz;
 }
 
 // Squared gap between a point and an axis-aligned box (0 inside).
@@ -682,16 +819,13 @@ __device__ __forceinline__ void contact_candidates(const ContactArgs& a, const i
 // search above would leave n/32 warps walking all n elements one after the other.  Here a warp
 // owns (group of 32 elements i, chunk of `cg` candidate groups) and writes its own slab
 // out[chunk][i]; the update kernel adds the slabs in chunk order.
-__global__ void __launch_bounds__(kThreads)
-nb_contact_chunk_kernel(const __grid_constant__ ContactArgs a, const int cg, const int nchunks)
+// The work of warp `wid` of that grid; cand [kCandCap], stage [kGroup], hq [kHitCap * 32]: the warp's shared memory.
+__device__ __forceinline__ void contact_chunk_warp(const ContactArgs& a, const int cg, const int nchunks, const int wid,
+                                                   int* __restrict__ cand, float4* __restrict__ stage,
+                                                   uint32_t* __restrict__ hq)
 {
-    __shared__ int cand_s[kThreads / 32][kCandCap];
-    __shared__ float4 stage_s[kThreads / 32][kGroup];
-    __shared__ uint32_t hit_s[kThreads / 32][kHitCap * 32];
-    const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-    uint32_t* hq = hit_s[wib];
+    const int lane = threadIdx.x & 31;
     int nh = 0;
-    const int wid = (blockIdx.x * kThreads + threadIdx.x) >> 5;
     const int ig = wid / nchunks, ch = wid - ig * nchunks;
     if (ig >= a.ngroups) return;
     const int k = ig * kGroup + lane;
@@ -703,12 +837,22 @@ nb_contact_chunk_kernel(const __grid_constant__ ContactArgs a, const int cg, con
     for (int gb = g0; gb < g1; gb += kCandCap) {
         const int cnt = min(kCandCap, g1 - gb);
         __syncwarp();
-        for (int q = lane; q < cnt; q += 32) cand_s[wib][q] = gb + q;
+        for (int q = lane; q < cnt; q += 32) cand[q] = gb + q;
         __syncwarp();
-        contact_candidates(a, cand_s[wib], cnt, stage_s[wib], hq, nh, pi, vi, valid, lane, ax, ay, az);
+        contact_candidates(a, cand, cnt, stage, hq, nh, pi, vi, valid, lane, ax, ay, az);
     }
     contact_drain(a, hq, nh, pi, vi, lane, ax, ay, az);
     if (valid) a.out[(size_t)ch * a.n + k] = make_float4((float)ax, (float)ay, (float)az, 0.f);
+}
+
+__global__ void __launch_bounds__(kThreads)
+nb_contact_chunk_kernel(const __grid_constant__ ContactArgs a, const int cg, const int nchunks)
+{
+    __shared__ int cand_s[kThreads / 32][kCandCap];
+    __shared__ float4 stage_s[kThreads / 32][kGroup];
+    __shared__ uint32_t hit_s[kThreads / 32][kHitCap * 32];
+    const int wib = threadIdx.x >> 5;
+    contact_chunk_warp(a, cg, nchunks, (blockIdx.x * kThreads + threadIdx.x) >> 5, cand_s[wib], stage_s[wib], hit_s[wib]);
 }
 
 // ---------------------------------------------------------------------------
@@ -718,7 +862,7 @@ nb_contact_chunk_kernel(const __grid_constant__ ContactArgs a, const int cg, con
 //   v_i += kick_h * a_i ;  x_i += drift_dt * v_i        (either may be 0)
 //   if advance: step += 1, R_s = ramp(step)             (expanding-star rule)
 struct UpdateArgs {
-    const float4* __restrict__ src;    // [nsrc][n]
+    const float4* src;                 // [nsrc][n]
     float4* acc_out;                   // may be null; may alias src when nsrc == 1
     float4* posm;
     float4* vel;
@@ -731,19 +875,56 @@ struct UpdateArgs {
 
 // Expanding-star rule (A8): step count n and R_s(n), linear in n over n_ramp steps, evaluated
 // in fp64 with explicit roundings (no contraction) and rounded once to the fp32 model parameter.
+__device__ __forceinline__ float ramp_radius(double R_start, double R_end, long long n_ramp, long long nstep)
+{
+    double Rs = R_start;
+    if (n_ramp > 0) {
+        const long long nn = nstep < n_ramp ? nstep : n_ramp;
+        Rs = __dadd_rn(R_start, __ddiv_rn(__dmul_rn(__dsub_rn(R_end, R_start), (double)nn), (double)n_ramp));
+    }
+    return (float)Rs;
+}
+
 __device__ __forceinline__ void set_step(DevState* d, long long nstep)
 {
     d->step = nstep;
-    for (int s = 0; s < 2; ++s) {
-        double Rs = d->R_start[s];
-        if (d->n_ramp > 0) {
-            const long long nn = nstep < d->n_ramp ? nstep : d->n_ramp;
-            Rs = __dadd_rn(d->R_start[s],
-                           __ddiv_rn(__dmul_rn(__dsub_rn(d->R_end[s], d->R_start[s]), (double)nn),
-                                     (double)d->n_ramp));
+    for (int s = 0; s < 2; ++s) d->R[s] = ramp_radius(d->R_start[s], d->R_end[s], d->n_ramp, nstep);
+}
+
+// Element i of the update, given a_i: kick, drift (new position and velocity through p, v: valid if moved).
+__device__ __forceinline__ void apply_update(const UpdateArgs& u, const int i, const float ax, const float ay, const float az,
+                                             float4& p, float4& v)
+{
+    if (u.acc_out) u.acc_out[i] = make_float4(ax, ay, az, 0.f);
+    if (u.kick_h != 0.f || u.drift_dt != 0.f || u.vscale != 1.f) {
+        v = u.vel[i];
+        v.x = fmaf(u.kick_h, ax, v.x);
+        v.y = fmaf(u.kick_h, ay, v.y);
+        v.z = fmaf(u.kick_h, az, v.z);
+        if (u.vscale != 1.f) { v.x *= u.vscale; v.y *= u.vscale; v.z *= u.vscale; }
+        u.vel[i] = v;
+        if (u.drift_dt != 0.f) {
+            p = u.posm[i];
+            p.x = fmaf(u.drift_dt, v.x, p.x);
+            p.y = fmaf(u.drift_dt, v.y, p.y);
+            p.z = fmaf(u.drift_dt, v.z, p.z);
+            u.posm[i] = p;
         }
-        d->R[s] = (float)Rs;
     }
+}
+
+// Element i of the update: a_i = sum of the slabs in slab order (fp64), then kick and drift.  Returns a_i.
+__device__ __forceinline__ float4 update_element(const UpdateArgs& u, const int i, float4& p, float4& v)
+{
+    double sx = 0.0, sy = 0.0, sz = 0.0;
+#pragma unroll 8
+    for (int q = 0; q < u.nsrc; ++q) {
+        const float4 t = u.src[(size_t)q * u.n + i];
+        sx += (double)t.x; sy += (double)t.y; sz += (double)t.z;
+    }
+    const float ax = (float)sx, ay = (float)sy, az = (float)sz;
+    apply_update(u, i, ax, ay, az, p, v);
+    return make_float4(ax, ay, az, 0.f);
 }
 
 __global__ void __launch_bounds__(256)
@@ -751,28 +932,8 @@ nb_reduce_update_kernel(const __grid_constant__ UpdateArgs u)
 {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < u.n) {
-        double sx = 0.0, sy = 0.0, sz = 0.0;
-        for (int p = 0; p < u.nsrc; ++p) {
-            const float4 q = u.src[(size_t)p * u.n + i];
-            sx += (double)q.x; sy += (double)q.y; sz += (double)q.z;
-        }
-        const float ax = (float)sx, ay = (float)sy, az = (float)sz;
-        if (u.acc_out) u.acc_out[i] = make_float4(ax, ay, az, 0.f);
-        if (u.kick_h != 0.f || u.drift_dt != 0.f || u.vscale != 1.f) {
-            float4 v = u.vel[i];
-            v.x = fmaf(u.kick_h, ax, v.x);
-            v.y = fmaf(u.kick_h, ay, v.y);
-            v.z = fmaf(u.kick_h, az, v.z);
-            if (u.vscale != 1.f) { v.x *= u.vscale; v.y *= u.vscale; v.z *= u.vscale; }
-            u.vel[i] = v;
-            if (u.drift_dt != 0.f) {
-                float4 p = u.posm[i];
-                p.x = fmaf(u.drift_dt, v.x, p.x);
-                p.y = fmaf(u.drift_dt, v.y, p.y);
-                p.z = fmaf(u.drift_dt, v.z, p.z);
-                u.posm[i] = p;
-            }
-        }
+        float4 p, v;
+        update_element(u, i, p, v);
     }
     if (u.advance && blockIdx.x == 0 && threadIdx.x == 0) set_step(u.dev, u.dev->step + 1);
 }

@@ -43,7 +43,7 @@ sm = bench.reduce_over_ranks(1.0 + rank, "sum")
 print(f"RESULT {{rank}} {{world}} {{mx}} {{sm}}", flush=True)
 # rank-0-only reference arm: other ranks exit 0 without work
 if rank != 0:
-    class A: gpus=2; steps=1; warmup=1
+    class A: gpus=2; steps=1; warmup=1; config=4
     assert bench.run_reference(A) == 0
 import torch.distributed as dist
 dist.destroy_process_group()
@@ -66,3 +66,26 @@ def test_two_rank_gloo_timing_reduction(tmp_path):
         res = [l for l in so.splitlines() if l.startswith("RESULT")][0].split()
         assert int(res[1]) == r and int(res[2]) == 2
         assert float(res[3]) == 15.0 and float(res[4]) == 3.0        # max over ranks, sum over ranks
+
+
+def test_gpus_flag_starts_the_ranks_itself():
+    """`python bench.py --gpus 2` with no launcher around it: bench.py starts two ranks (RANK / WORLD_SIZE / MASTER_*
+    as torchrun would), they rendezvous (gloo here: the GPU is taken out of the timing path by --impl stub), the
+    timing is the max over ranks, the units the sum, and rank 0 alone prints, with n_gpus = 2."""
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "stub", "--steps", "4"],
+                         capture_output=True, text=True, env=env, cwd=ROOT, timeout=600)
+    assert out.returncode == 0, out.stderr
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1                                   # rank 0 only
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["steps"] == 4 and d["config"]["parallelism"] == "replicas only"
+    assert d["ms_per_step"] >= 3.9                           # rank 1 sleeps 4 ms per step, rank 0 only 2: the max over ranks
+    assert abs(d["value"] - 2 * 1000.0 / (d["ms_per_step"] * 1e-3)) < 1e-6 * d["value"]   # units of BOTH ranks / that time
+
+
+def test_gpus_flag_must_agree_with_the_launcher():
+    env = dict(os.environ, RANK="0", LOCAL_RANK="0", WORLD_SIZE="1", MASTER_ADDR="127.0.0.1", MASTER_PORT="29618")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "stub"],
+                         capture_output=True, text=True, env=env, cwd=ROOT, timeout=600)
+    assert out.returncode != 0 and "WORLD_SIZE=1" in (out.stderr + out.stdout)

@@ -278,10 +278,21 @@ def test_bench_line_has_the_contract_keys(nb):
     assert d["higher_is_better"] is True and d["dtype"] == "f32" and d["data"] == "synthetic" and d["vs_baseline"] is None
     assert d["config"]["workload"].startswith("config4") and d["config"]["n"] == 262144
     assert d["value"] > 1e12 and abs(d["value"] - 262144.0 ** 2 / (d["ms_per_step"] * 1e-3)) < 1e-6 * d["value"]
+    assert d["ms_per_step_best"] <= d["ms_per_step_median"] <= 1.2 * d["ms_per_step"]
+    assert abs(d["pct_of_fp32_peak_20flop"] / d["pct_of_fp32_peak"] - 20.0 / 21.0) < 1e-9
     r = d["roofline"]
-    assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and 0.3 < r["frac"] < 1.2 and r["frac_executed"] < r["frac"]
+    # frac is what the ALUs executed (< 1); the algorithmic 21-flop figure sits beside it and may reach 1
+    assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and 0.3 < r["frac"] < 0.9 and r["frac"] < r["frac_algorithmic"] < 1.2
+    assert 0.3 < r["fma_pipe_frac"] < 1.0 and 0.3 < r["xu_pipe_frac"] < 1.0
     assert r["kernel"].startswith("nb_gravity_sym_kernel<1024") and 0.9 < r["kernel_share_of_step"] <= 1.0
     assert abs(r["achieved"] / r["peak"] - r["frac"]) < 1e-9
+    assert r["traffic"] is None or r["traffic"] > 0
     e = d["e2e"]
     assert e["h2d_bytes_per_step"] == e["d2h_bytes_per_step"] == 3 * 262144 * 16 and 0 < e["value"] < d["value"]
     assert d["gpu_launches"] >= 3 * 3 and d["clocks"]["sm_mhz"] > 0
+    pc = {c["workload"].split("_")[0]: c for c in d["per_config"]}
+    assert sorted(pc) == ["config1", "config2", "config3", "config5"]
+    for c in pc.values():
+        assert c["ms_per_step_best"] <= c["ms_per_step_median"] and c["interactions_per_s"] > 1e10 and c["ms_per_step_hot"] > 0
+        assert abs(c["interactions_per_s"] - float(c["n"]) ** 2 / (c["ms_per_step"] * 1e-3)) < 1e-6 * c["interactions_per_s"]
+    assert pc["config1"]["fused_one_launch"] and "sym" in pc["config3"]["kernel"] and "sym" in pc["config5"]["kernel"]

@@ -177,7 +177,7 @@ def test_default_path_and_both_paths_agree_at_full_size(nb):
     _check_accel(nb, w, p, rows=_sample(w.n, 1024, 5), force_path=nb.NB_PATH_ONE_SIDED)
 
 
-@pytest.mark.parametrize("n,name", [(24576, "<256"), (30001, "<256"), (32768, "<512"), (120000, "<1024"), (400000, "<2048")])
+@pytest.mark.parametrize("n,name", [(10240, "<256"), (24576, "<256"), (30001, "<256"), (32768, "<512"), (120000, "<1024"), (400000, "<2048")])
 def test_symmetric_tile_bands(nb, n, name):
     """Sizes in each super-tile band below config 5's (S = 256, 512, 1024, 2048; 4096 is config 5),
     ragged against the band's tile, sampled rows against the oracle."""
