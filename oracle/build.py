@@ -11,15 +11,20 @@ import subprocess
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 SRC = os.path.join(HERE, "nb_oracle.c")
-LIB = os.path.join(HERE, "libnb_oracle.so")
+# NB_ORACLE_SANITIZE=1: an AddressSanitizer + UndefinedBehaviorSanitizer build in its own file, for running the
+# pins under the sanitizers (LD_PRELOAD the gcc libasan.so into python; see profiles/r2_sanitizers.md)
+SANITIZE = os.environ.get("NB_ORACLE_SANITIZE", "") not in ("", "0")
+LIB = os.path.join(HERE, "libnb_oracle_asan.so" if SANITIZE else "libnb_oracle.so")
 
 
 def build(force: bool = False) -> str:
     if (not force and os.path.exists(LIB)
             and os.path.getmtime(LIB) >= os.path.getmtime(SRC)):
         return LIB
-    cmd = ["gcc", "-O2", "-std=c11", "-fopenmp", "-fPIC", "-shared",
-           "-ffp-contract=off", "-o", LIB, SRC, "-lm"]
+    opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer"] \
+        if SANITIZE else ["-O2"]
+    cmd = ["gcc"] + opt + ["-std=c11", "-fopenmp", "-fPIC", "-shared",
+                           "-ffp-contract=off", "-o", LIB, SRC, "-lm"]
     subprocess.check_call(cmd)
     return LIB
 

@@ -76,3 +76,51 @@ def test_steps_relax_and_diagnostics_small(n1, n2, path):
     nb.nb_set_step(s.ctx, 2)
     assert nb.nb_get_step(s.ctx)[0] == 2
     s.close()
+
+
+@pytest.mark.parametrize("n1,n2,path", [(700, 501, 0), (5200, 3101, 1), (5200, 3101, 2), (33, 0, 0)])
+def test_no_write_outside_the_callers_buffers(n1, n2, path):
+    """compute-sanitizer is closed on this pool (profiles/r2_sanitizers.md), so the library's writes are fenced in by
+    hand: every buffer it is given -- state, star, output, workspace, image -- is carved out of ONE allocation with 4 KB
+    guard zones of a known byte pattern on both sides, every entry point runs, and the guards must come back intact."""
+    import torch
+    import paper_2303_12166_b200 as nb
+    w = _w(max(n1, 1), max(n2, 1), 11)
+    n = n1 + n2
+    posm_h, vel_h, star_h = w.posm[:n].copy(), w.vel[:n].copy(), w.star[:n].copy()
+    p = params_f32(w.params)
+    dev = torch.device("cuda:0")
+    G, W, H = 4096, 40, 24
+    sizes = dict(posm=n * 16, vel=n * 16, star=n * 4, acc=n * 16, ws=nb.nb_workspace_bytes(n), img=2 * W * H * 4)
+    off, o = {}, G
+    for k, b in sizes.items():
+        o = (o + 255) // 256 * 256
+        off[k] = o
+        o += b + G
+    buf = torch.full((o + 256,), 0xA5, dtype=torch.uint8, device=dev)
+    base = (buf.data_ptr() + 255) // 256 * 256 - buf.data_ptr()          # 256-byte aligned start inside the tensor
+    view = lambda k: buf[base + off[k]: base + off[k] + sizes[k]]
+    view("posm").copy_(torch.as_tensor(posm_h).view(torch.uint8).reshape(-1))
+    view("vel").copy_(torch.as_tensor(vel_h).view(torch.uint8).reshape(-1))
+    view("star").copy_(torch.as_tensor(star_h).view(torch.uint8).reshape(-1))
+    ptr = lambda k: buf.data_ptr() + base + off[k]
+    ctx = nb.nb_create(n, p, torch.cuda.current_stream(dev).cuda_stream)
+    if path:
+        nb.nb_set_force_path(ctx, path)
+    nb.nb_set_state(ctx, n, ptr("posm"), ptr("vel"), ptr("star"), ptr("ws"), sizes["ws"])
+    nb.nb_compute_accel(ctx, ptr("acc"))
+    nb.nb_step(ctx, 3)
+    nb.nb_relax(ctx, 1, 2.0)
+    nb.nb_energy(ctx)
+    nb.nb_transfer_diagnostics(ctx)
+    nb.nb_splat(ctx, [0.0, 0.0, 0.0], 2.0, 0, 1, W, H, ptr("img"))
+    nb.nb_set_step(ctx, 1)
+    nb.nb_time_force_kernel(ctx, 1); nb.nb_time_contact_pass(ctx, 1)
+    torch.cuda.synchronize()
+    nb.nb_destroy(ctx)
+    inside = torch.zeros(buf.numel(), dtype=torch.bool, device=dev)
+    for k in sizes:
+        inside[base + off[k]: base + off[k] + sizes[k]] = True
+    assert bool((buf[~inside] == 0xA5).all()), "a kernel wrote outside the buffers it was given"
+    x = view("posm").view(torch.float32).reshape(n, 4)
+    assert bool(torch.isfinite(x).all()) and int(view("img").view(torch.int32).sum()) <= n
