@@ -242,11 +242,38 @@ bool params_ok(const nb_params* p)
 }
 
 // The instantiations of the symmetric kernel: <S, elements i per lane, threads, CTAs/SM, unroll>.
-#define NB_SYM_256  nb_gravity_sym_kernel<256, 4, 64, 8, 8>
-#define NB_SYM_512  nb_gravity_sym_kernel<512, 4, 128, 4, 8>
-#define NB_SYM_1024 nb_gravity_sym_kernel<1024, 4, 256, 2, 8>
-#define NB_SYM_2048 nb_gravity_sym_kernel<2048, 4, 256, 2, 8>
-#define NB_SYM_4096 nb_gravity_sym_kernel<4096, 4, 256, 2, 8>
+// 8 elements i per lane (254 registers, 8 warps per SM): a rotation step then carries 16 pair evaluations for its
+// 6 SHFL + 3 LDS, and all 8 pairs' MUFU are in flight together (measured at N = 262,144: 4 i per lane / 16 warps
+// 19.36 ms, 8 / 8 warps 18.41 ms, 8 / 12 warps at 168 registers 18.76 ms).
+template <int S> struct SymShape;
+template <> struct SymShape<256>  { static constexpr int NI = 4, NT = 64,  MINB = 8, UNR = 8; };   // small n: more, smaller CTAs win (16,384: 103 vs 113 us)
+template <> struct SymShape<512>  { static constexpr int NI = 8, NT = 64,  MINB = 4, UNR = 16; };
+template <> struct SymShape<1024> { static constexpr int NI = 8, NT = 128, MINB = 2, UNR = 16; };
+template <> struct SymShape<2048> { static constexpr int NI = 8, NT = 128, MINB = 2, UNR = 16; };
+template <> struct SymShape<4096> { static constexpr int NI = 8, NT = 128, MINB = 2, UNR = 16; };
+
+template <int S>
+int launch_sym(nb_ctx* c, const SymArgs& sa, int grid)
+{
+    using K = SymShape<S>;
+    auto kernel = nb_gravity_sym_kernel<S, K::NI, K::NT, K::MINB, K::UNR>;
+    static bool configured = false;                   // the kernel's shared memory is dynamic (112 KB at S = 4096)
+    if (!configured) {
+        NB_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * S));
+        configured = true;
+    }
+    kernel<<<grid, K::NT, kSymSmemPerElem * S, c->stream>>>(sa);
+    return NB_OK;
+}
+
+template <int S>
+const char* sym_name()
+{
+    using K = SymShape<S>;
+    static char buf[64];
+    std::snprintf(buf, sizeof(buf), "nb_gravity_sym_kernel<%d,%d,%d,%d,%d>", S, K::NI, K::NT, K::MINB, K::UNR);
+    return buf;
+}
 
 // Row a2: partial gravitational accelerations -> part[0..ngrav-1][n]
 //   symmetric kernel: one CTA per pair of super-tiles, part[Y][e] = a_e due to super-tile Y
@@ -259,12 +286,13 @@ int launch_gravity(nb_ctx* c)
         sa.G = c->prm.G; sa.eps = c->prm.eps;
         const long long T = c->plan.T;
         const int grid = (int)(T * (T + 1) / 2);
-        const int smem = kSymSmemPerElem * c->plan.sym_S;
-        if (c->plan.sym_S == 256)       NB_SYM_256<<<grid, 64, smem, c->stream>>>(sa);
-        else if (c->plan.sym_S == 512)  NB_SYM_512<<<grid, 128, smem, c->stream>>>(sa);
-        else if (c->plan.sym_S == 1024) NB_SYM_1024<<<grid, 256, smem, c->stream>>>(sa);
-        else if (c->plan.sym_S == 2048) NB_SYM_2048<<<grid, 256, smem, c->stream>>>(sa);
-        else                            NB_SYM_4096<<<grid, 256, smem, c->stream>>>(sa);
+        int rc;
+        if (c->plan.sym_S == 256)       rc = launch_sym<256>(c, sa, grid);
+        else if (c->plan.sym_S == 512)  rc = launch_sym<512>(c, sa, grid);
+        else if (c->plan.sym_S == 1024) rc = launch_sym<1024>(c, sa, grid);
+        else if (c->plan.sym_S == 2048) rc = launch_sym<2048>(c, sa, grid);
+        else                            rc = launch_sym<4096>(c, sa, grid);
+        if (rc) return rc;
         c->launches++;
         NB_CUDA(c, cudaGetLastError());
         return NB_OK;
@@ -488,14 +516,6 @@ int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
         if (coop && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, nb_fused_step_kernel, kThreads, 0) == cudaSuccess)
             c->fused_blocks = per_sm * c->num_sms;
-    }
-    // the symmetric kernel's shared memory is dynamic (112 KB at S = 4096)
-    if (cudaFuncSetAttribute(NB_SYM_512, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 512) != cudaSuccess ||
-        cudaFuncSetAttribute(NB_SYM_1024, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 1024) != cudaSuccess ||
-        cudaFuncSetAttribute(NB_SYM_2048, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 2048) != cudaSuccess ||
-        cudaFuncSetAttribute(NB_SYM_4096, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * 4096) != cudaSuccess) {
-        nb_destroy(c);
-        return NB_ECUDA;
     }
     *out = c;
     return NB_OK;
@@ -816,11 +836,11 @@ int nb_set_force_path(nb_ctx* c, int path)
 const char* nb_force_kernel_name(nb_ctx* c)
 {
     if (!c || !c->have_state) return "";
-    if (c->plan.sym_S == 256) return "nb_gravity_sym_kernel<256,4,64,8,8>";
-    if (c->plan.sym_S == 512) return "nb_gravity_sym_kernel<512,4,128,4,8>";
-    if (c->plan.sym_S == 1024) return "nb_gravity_sym_kernel<1024,4,256,2,8>";
-    if (c->plan.sym_S == 2048) return "nb_gravity_sym_kernel<2048,4,256,2,8>";
-    if (c->plan.sym_S) return "nb_gravity_sym_kernel<4096,4,256,2,8>";
+    if (c->plan.sym_S == 256) return sym_name<256>();
+    if (c->plan.sym_S == 512) return sym_name<512>();
+    if (c->plan.sym_S == 1024) return sym_name<1024>();
+    if (c->plan.sym_S == 2048) return sym_name<2048>();
+    if (c->plan.sym_S) return sym_name<4096>();
     return c->plan.TJ == 256 ? "nb_gravity_kernel<2,256>" : "nb_gravity_kernel<2,128>";
 }
 

@@ -366,8 +366,8 @@ nb_gravity_kernel(const __grid_constant__ GravArgs a)
 // finished reaction sums of pair l over the warp's 32 NI elements i and adds them to the CTA's
 // shared-memory array.  The warps of a CTA are skewed over different tiles and meet at a barrier
 // after every tile, so the shared-memory sums have a fixed order: bitwise reproducible.
-// Per lane and step at NI = 4 (4 i x 2 j = 8 pairs = 16 interactions): 60 packed FP32 instructions
-// (FADD2 x12, FFMA2 x12+4, FMUL2 x8, FFMA2 x12+12), 16 MUFU (one RSQ and one RCP per pair: a pair
+// Per lane and step at NI = 8 (8 i x 2 j = 16 pairs = 32 interactions): 120 packed FP32 instructions
+// (FADD2 x24, FFMA2 x24+8, FMUL2 x16, FFMA2 x24+24), 32 MUFU (one RSQ and one RCP per pair: a pair
 // evaluation already serves two interactions, so the shared reciprocal of the one-sided kernel
 // would cost more FMA-pipe cycles than the XU cycles it saves), 6 SHFL, 3 LDS.64 -- 13.5 executed
 // flop per interaction against 22 one-sided.  DESIGN.md 5.1c lists the variants measured on the way
@@ -377,7 +377,8 @@ nb_gravity_kernel(const __grid_constant__ GravArgs a)
 // one-sided loop).  Super-tiles of one mass take the mass out of the loop, as in
 // the one-sided kernel; other pairs of super-tiles multiply c by G m_j and G m_i per pair.
 // Template parameters: S super-tile, NI elements i per lane, NT threads, MINB CTAs/SM, UNR unroll
-// of the 32-step rotation (shipped: 8).  A step is written phase by phase over the NI elements i
+// of the 32-step rotation (shipped: 8 i per lane, 128 threads, 2 CTAs/SM, unroll 16 at S >= 512: 254 registers,
+// 8 warps per SM).  A step is written phase by phase over the NI elements i
 // (d and r^2 of all, then all MUFU.RSQ, ...), which keeps the MUFU of all of them in flight together.
 struct SymArgs {
     const float4* __restrict__ posm;   // [n] x,y,z,m
@@ -388,6 +389,10 @@ struct SymArgs {
 
 constexpr int kSymSmemPerElem = 28;    // dynamic shared memory of the symmetric kernel: (16 + 3*4) bytes x S
 
+#ifndef NB_SYM_GROUP
+#define NB_SYM_GROUP 8       // elements i whose phases are interleaved (all d and r^2, then all MUFU.RSQ, ...)
+#endif
+
 template <int NI, bool UNI, bool SYM>
 __device__ __forceinline__ void sym_step(const f32x2 X, const f32x2 Y, const f32x2 Z, const f32x2 M,
                                          const float (&nxi)[NI], const float (&nyi)[NI], const float (&nzi)[NI],
@@ -395,47 +400,55 @@ __device__ __forceinline__ void sym_step(const f32x2 X, const f32x2 Y, const f32
                                          f32x2 (&ax)[NI], f32x2 (&ay)[NI], f32x2 (&az)[NI],
                                          f32x2& jx, f32x2& jy, f32x2& jz)
 {
+    constexpr int GI = NI < NB_SYM_GROUP ? NI : NB_SYM_GROUP;
+    static_assert(NI % GI == 0, "whole groups of elements i");
     const f32x2 tiny2 = pk2(kTinyR2, kTinyR2);
-    f32x2 dx[NI], dy[NI], dz[NI], r2[NI], ri[NI], t[NI], c[NI];
-    // phase by phase over the NI elements i, so that the MUFU of all of them are in flight together
 #pragma unroll
-    for (int i = 0; i < NI; ++i) {
-        dx[i] = add2(X, pk2(nxi[i], nxi[i])); dy[i] = add2(Y, pk2(nyi[i], nyi[i])); dz[i] = add2(Z, pk2(nzi[i], nzi[i]));
-        r2[i] = fma2(dx[i], dx[i], tiny2); r2[i] = fma2(dy[i], dy[i], r2[i]); r2[i] = fma2(dz[i], dz[i], r2[i]);
-    }
+    for (int g = 0; g < NI; g += GI) {
+        f32x2 dx[GI], dy[GI], dz[GI], r2[GI], ri[GI], t[GI], c[GI];
+        // phase by phase over the GI elements i, so that the MUFU of all of them are in flight together
 #pragma unroll
-    for (int i = 0; i < NI; ++i) {
-        float a0, b0;
-        unpk2(r2[i], a0, b0);
-        ri[i] = pk2(rsqrt_approx(a0), rsqrt_approx(b0));                   // 1/r
-    }
+        for (int i = 0; i < GI; ++i) {
+            dx[i] = add2(X, pk2(nxi[g + i], nxi[g + i])); dy[i] = add2(Y, pk2(nyi[g + i], nyi[g + i]));
+            dz[i] = add2(Z, pk2(nzi[g + i], nzi[g + i]));
+            r2[i] = fma2(dx[i], dx[i], tiny2); r2[i] = fma2(dy[i], dy[i], r2[i]); r2[i] = fma2(dz[i], dz[i], r2[i]);
+        }
 #pragma unroll
-    for (int i = 0; i < NI; ++i) {
-        const f32x2 sm = fma2(r2[i], ri[i], eps2);                         // r + eps
-        t[i] = mul2(sm, sm);                                               // (r + eps)^2
-    }
+        for (int i = 0; i < GI; ++i) {
+            float a0, b0;
+            unpk2(r2[i], a0, b0);
+            ri[i] = pk2(rsqrt_approx(a0), rsqrt_approx(b0));                   // 1/r
+        }
 #pragma unroll
-    for (int i = 0; i < NI; ++i) {
-        float a0, b0;
-        unpk2(t[i], a0, b0);
-        c[i] = mul2(ri[i], pk2(rcp_approx(a0), rcp_approx(b0)));           // 1/(r (r+eps)^2)   Eq. 4
-    }
+        for (int i = 0; i < GI; ++i) {
+            const f32x2 sm = fma2(r2[i], ri[i], eps2);                         // r + eps
+            t[i] = mul2(sm, sm);                                               // (r + eps)^2
+        }
 #pragma unroll
-    for (int i = 0; i < NI; ++i) {
-        if (UNI) {
-            if (SYM) {
-                ax[i] = fma2v(c[i], dx[i], ax[i]); jx = fma2v(c[i], dx[i], jx);
-                ay[i] = fma2v(c[i], dy[i], ay[i]); jy = fma2v(c[i], dy[i], jy);
-                az[i] = fma2v(c[i], dz[i], az[i]); jz = fma2v(c[i], dz[i], jz);
+        for (int i = 0; i < GI; ++i) {
+            float a0, b0;
+            unpk2(t[i], a0, b0);
+            c[i] = mul2(ri[i], pk2(rcp_approx(a0), rcp_approx(b0)));           // 1/(r (r+eps)^2)   Eq. 4
+        }
+#pragma unroll
+        for (int i = 0; i < GI; ++i) {
+            if (UNI) {
+                if (SYM) {
+                    ax[g + i] = fma2v(c[i], dx[i], ax[g + i]); jx = fma2v(c[i], dx[i], jx);
+                    ay[g + i] = fma2v(c[i], dy[i], ay[g + i]); jy = fma2v(c[i], dy[i], jy);
+                    az[g + i] = fma2v(c[i], dz[i], az[g + i]); jz = fma2v(c[i], dz[i], jz);
+                } else {
+                    ax[g + i] = fma2(c[i], dx[i], ax[g + i]); ay[g + i] = fma2(c[i], dy[i], ay[g + i]);
+                    az[g + i] = fma2(c[i], dz[i], az[g + i]);
+                }
             } else {
-                ax[i] = fma2(c[i], dx[i], ax[i]); ay[i] = fma2(c[i], dy[i], ay[i]); az[i] = fma2(c[i], dz[i], az[i]);
-            }
-        } else {
-            const f32x2 ci = mul2(c[i], M);                                // G m_j for a_i
-            ax[i] = fma2(ci, dx[i], ax[i]); ay[i] = fma2(ci, dy[i], ay[i]); az[i] = fma2(ci, dz[i], az[i]);
-            if (SYM) {
-                const f32x2 cj = mul2(c[i], pk2(gmi[i], gmi[i]));          // G m_i for a_j
-                jx = fma2(cj, dx[i], jx); jy = fma2(cj, dy[i], jy); jz = fma2(cj, dz[i], jz);
+                const f32x2 ci = mul2(c[i], M);                                // G m_j for a_i
+                ax[g + i] = fma2(ci, dx[i], ax[g + i]); ay[g + i] = fma2(ci, dy[i], ay[g + i]);
+                az[g + i] = fma2(ci, dz[i], az[g + i]);
+                if (SYM) {
+                    const f32x2 cj = mul2(c[i], pk2(gmi[g + i], gmi[g + i]));  // G m_i for a_j
+                    jx = fma2(cj, dx[i], jx); jy = fma2(cj, dy[i], jy); jz = fma2(cj, dz[i], jz);
+                }
             }
         }
     }
