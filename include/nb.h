@@ -16,14 +16,16 @@
  *   - "dev" pointers are CUDA device pointers on the device that was current
  *     at nb_create(); "host" pointers are ordinary host memory.
  *   - The CALLER owns every device byte (state, output, workspace).  The
- *     library owns only the host-side nb_ctx (plus one internal stream and two events) and
- *     never allocates device memory.
+ *     library owns only the host-side nb_ctx (plus one internal stream and two events: SURVEY 8(b) says
+ *     "owns only the host-side nb_ctx" -- the stream carries the contact pass beside the gravity kernel and
+ *     is created and destroyed with the ctx) and never allocates device memory.
  *     Borrowed pointers must stay valid until the next nb_set_state()/nb_destroy().
  *   - All device work is ordered on the borrowed stream given to nb_create() (the contact
  *     pass runs on a library-owned non-blocking stream, forked from and joined back into the
  *     borrowed stream by events inside each force evaluation -- invisible to the caller).
- *     Nothing synchronises except nb_set_state(), nb_energy() and
- *     nb_download_state().  One ctx per host thread.
+ *     Nothing synchronises except nb_set_state() (SURVEY 8(b) lists only nb_energy(); binding has to
+ *     read back the verdict on star[] before it can return NB_ESTATE), nb_energy(), nb_get_step(),
+ *     nb_transfer_diagnostics() and nb_download_state().  One ctx per host thread.
  *   - Element layout: elements of star 0 first, then star 1.  posm[i] =
  *     (x, y, z, m_i), vel[i] = (vx, vy, vz, unused); both float4, 16-byte aligned.
  *
@@ -77,12 +79,11 @@ typedef struct {
  * current device has compute capability 10.x. */
 int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream);
 
-/* Bytes of device workspace nb_set_state() needs for a context of n_max elements
- * (cached acceleration, partial sums of the gravity kernel -- up to 513 slabs of n float4 for the
- * symmetric kernel: 2-8 KB per element, 1.0 GiB at n_max = 262144, 4.6 GiB at 1048576 --, device-side
- * step/radius state,
- * reduction scratch, and the contact pass's Hilbert keys, sort scratch, ordered copy and
- * group boxes).  0 if n_max is out of range. */
+/* Bytes of device workspace nb_set_state() needs for a context of n_max elements: cached acceleration,
+ * the gravity kernel's partial sums (slabs of n float4 for n < 98304; from there on the symmetric kernel adds
+ * into two fp64 sums per element instead), device-side step/radius state, reduction scratch, and the contact
+ * pass's cell table, counting-sort buffers and ordered copy.  3 MiB at n_max = 2048, 134 MiB at 65536,
+ * 322 MiB at 262144, 419 MiB at 1048576.  0 if n_max is out of range. */
 size_t nb_workspace_bytes(int64_t n_max);
 
 /* Bind the state.  posm, vel: dev float[n][4], 16-byte aligned, BORROWED and
@@ -168,16 +169,21 @@ int nb_download_state(nb_ctx* ctx, float* host_posm, float* host_vel, float* hos
 int nb_get_launch_info(nb_ctx* ctx, int32_t* out4);
 
 /* Which kernel evaluates row a2 (Eq. 4, summed over all pairs).
- *   NB_PATH_AUTO (default): the symmetric kernel for 10240 <= n <= 2097152, else the one-sided
- *     kernel (the symmetric kernel is never used above 2097152 elements: its partial sums would
- *     not fit; NB_PATH_SYMMETRIC then falls back to the one-sided kernel as well).
+ *   NB_PATH_AUTO (default): the symmetric kernel for n >= 10240, else the one-sided kernel (n < 8192:
+ *     inside one fused launch per nb_step() call).
  *   NB_PATH_ONE_SIDED: every ORDERED pair (i, j) is evaluated; a CTA owns an (i-block, j-split).
  *   NB_PATH_SYMMETRIC: every UNORDERED pair is evaluated once and serves both a_i and a_j
  *     (the force of Eq. 4 is "between elements i and j": F_ij = -F_ji); a CTA owns a pair of
  *     super-tiles.  Both compute the same sum in a fixed order (bitwise reproducible run to run);
  *     they differ from each other by fp32 rounding only.
  * May be called before or after nb_set_state(); NB_ENOMEM if the bound workspace cannot hold the
- * partial sums of the requested path for the bound n (it always can for the default path).  Drops nothing: the cached acceleration stays valid. */
+ * partial sums of the requested path for the bound n (it always can for the default path).  Drops nothing: the
+ * cached acceleration stays valid.
+ * For n >= 98304 the symmetric kernel runs in "chain mode": its CTAs add their results into one pair of fp64 sums per
+ * element, super-tile by super-tile in a fixed order kept by turn counters (still bitwise reproducible, no atomics
+ * on data).  Should a turn ever fail to come (it cannot by construction; the check keeps a bug from hanging the GPU),
+ * the next synchronising call (nb_energy, nb_get_step, nb_download_state) returns NB_ECUDA with
+ * nb_last_cuda_error() == cudaErrorLaunchTimeout. */
 enum { NB_PATH_AUTO = 0, NB_PATH_ONE_SIDED = 1, NB_PATH_SYMMETRIC = 2 };
 int nb_set_force_path(nb_ctx* ctx, int path);
 

@@ -30,6 +30,7 @@ struct Plan {           // launch configuration of the gravity kernel for a give
     int nsplit = 1;     // j splits P
     int sym_S = 0;      // > 0: symmetric kernel with super-tiles of sym_S elements (else the one-sided kernel)
     int T = 0;          // symmetric kernel: number of super-tiles = slabs of partial sums
+    bool chain = false; // symmetric kernel in chain mode: two fp64 accumulators per element instead of the T slabs
 };
 
 constexpr int kCtasPerSM = 8;                      // resident CTAs/SM of nb_gravity_kernel<2, .> (64 registers)
@@ -48,7 +49,9 @@ constexpr int64_t kSymMinN = 10240;               // auto: symmetric kernel from
                                                   // beside it; measured whole steps (one-sided / symmetric, us): 8,192: 64 / 67,
                                                   // 10,240: 79 / 78, 12,288: 105 / 89, 16,384: 164 / 137, 24,576: 331 / 243
 constexpr int64_t kSym256MaxN = 32768;             // below this the super-tiles are 256 elements (CTAs of 2 warps)
-constexpr int64_t kSymMaxN = (int64_t)1 << 21;    // ... up to here: its T slabs of n float4 reach 17 GB at 2M elements
+constexpr int64_t kSymMaxN = (int64_t)1 << 26;    // ... for every n the library takes
+constexpr int64_t kChainMinN = 98304;             // from here on (S >= 1,024) the symmetric kernel runs in chain mode: its T
+                                                  // slabs would be 1.1 GB at 262,144 elements and 5 GB at 1,048,576
 
 // Super-tile size of the symmetric kernel for n elements: its T = ceil(n/S) slabs of n float4
 // partial sums cost memory and one extra pass, so S grows with n.
@@ -57,8 +60,8 @@ int sym_tile(int64_t n)
     if (n < kSym256MaxN) return 256;  // small n: more, smaller CTAs (T <= 128)
     if (n < 98304) return 512;        // T <= 192
     if (n < 393216) return 1024;      // T <= 384
-    if (n < 786432) return 2048;      // T <= 384
-    return 4096;
+    if (n < 786432) return 2048;
+    return 4096;                      // (chain mode keeps no slabs; measured at 1,048,576: S = 2,048 299.3 ms, 4,096 299.0)
 }
 
 int64_t sym_slabs(int64_t n) { const int64_t S = sym_tile(n); return (n + S - 1) / S; }
@@ -99,10 +102,11 @@ int64_t partial_elems_bound(int64_t n_max)
     const int64_t b = b1 > b2 ? b1 : b2;
     int64_t r = a < b ? a : b;
     // symmetric kernel: (T(n) + 1) n, largest just below each change of the super-tile size
-    const int64_t top = n_max < kSymMaxN ? n_max : kSymMaxN;
-    const int64_t tops[4] = {kSym256MaxN - 1, 98303, 393215, 786431};
-    int64_t probes[5] = {top, top, top, top, top};
-    for (int k = 0; k < 4; ++k) if (tops[k] < top) probes[k + 1] = tops[k];
+    // (only below kChainMinN: chain mode keeps two fp64 sums per element instead)
+    const int64_t top = n_max < kChainMinN - 1 ? n_max : kChainMinN - 1;
+    const int64_t tops[1] = {kSym256MaxN - 1};
+    int64_t probes[2] = {top, top};
+    for (int k = 0; k < 1; ++k) if (tops[k] < top) probes[k + 1] = tops[k];
     for (int64_t n : probes) {
         const int64_t e = (sym_slabs(n) + contact_slabs(n)) * n;
         if (e > r) r = e;
@@ -119,6 +123,7 @@ Plan make_plan(int64_t n, int num_sms, int path)
     if ((path == kPathSymmetric || (path == kPathAuto && n >= kSymMinN)) && n <= kSymMaxN) {
         p.sym_S = sym_tile(n);
         p.T = (int)sym_slabs(n);
+        p.chain = n >= kChainMinN;
     }
     p.I = 2;
     p.TJ = n >= 16384 ? 256 : 128;
@@ -141,7 +146,7 @@ Plan make_plan(int64_t n, int num_sms, int path)
 
 struct Layout {
     size_t off_dev, off_acc, off_part, off_red, off_ps, off_vs, off_gbox, off_sbox, off_cpart, off_cstate,
-        off_counters, off_bsum, off_bucket, off_slot, off_tmp, off_perm, total;
+        off_counters, off_bsum, off_bucket, off_slot, off_tmp, off_perm, off_acc64, off_turn, total;
 };
 
 // cell_cap(n1) + cell_cap(n - n1) < 4 n + 128 for every split of n <= n_max elements
@@ -172,6 +177,8 @@ Layout make_layout(int64_t n_max)
     L.off_slot = o;     o += align_up((size_t)n_max * sizeof(int));
     L.off_tmp = o;      o += align_up((size_t)n_max * sizeof(int));
     L.off_perm = o;     o += align_up((size_t)n_max * sizeof(uint32_t));
+    L.off_acc64 = o;    o += align_up(n_max >= kChainMinN ? (size_t)n_max * 6 * sizeof(double) : 0);
+    L.off_turn = o;     o += align_up(n_max >= kChainMinN ? ((size_t)(n_max / 1024 + 1) * 5 + 2) * sizeof(int) : 0);   // <= 4 rounds + 1 per tile
     L.total = o;
     return L;
 }
@@ -193,6 +200,7 @@ struct nb_ctx {
     Layout lay{};
     Plan plan{};
     bool have_state = false, have_acc = false;
+    bool chain_launched = false;          // the turn counters / error flag of chain mode hold a launch's state
     int path = kPathAuto;
     int last_cuda = 0;
     int64_t launches = 0;
@@ -207,7 +215,7 @@ struct nb_ctx {
     float4* sbox() const { return reinterpret_cast<float4*>(ws + lay.off_sbox); }
     template <class T> T* at(size_t off) const { return reinterpret_cast<T*>(ws + off); }
     bool contact_on() const { return prm.gamma > 0.f; }
-    int ngrav() const { return plan.sym_S ? plan.T : plan.nsplit; }       // gravity slabs
+    int ngrav() const { return plan.sym_S ? (plan.chain ? 0 : plan.T) : plan.nsplit; }   // gravity slabs
     int ncontact() const {                                                // contact slabs
         if (!contact_on()) return 0;
         return contact_slabs(n);
@@ -253,26 +261,43 @@ template <> struct SymShape<2048> { static constexpr int NI = 8, NT = 128, MINB 
 template <> struct SymShape<4096> { static constexpr int NI = 8, NT = 128, MINB = 2, UNR = 16; };
 
 template <int S>
-int launch_sym(nb_ctx* c, const SymArgs& sa, int grid)
+int launch_sym(nb_ctx* c, SymArgs& sa, int grid)
 {
     using K = SymShape<S>;
+    const int smem = kSymSmemPerElem * S;
+    if (c->plan.chain) {                              // nb_kernels.cuh "Chain mode"
+        auto kernel = nb_gravity_sym_chain_kernel<S, K::NI, K::NT, K::MINB, K::UNR>;
+        static bool configured = false;
+        if (!configured) {
+            NB_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            configured = true;
+        }
+        sa.acc64 = c->template at<double>(c->lay.off_acc64);
+        sa.turn = c->template at<int>(c->lay.off_turn);
+        constexpr int kRounds = S / (K::NT * K::NI);
+        NB_CUDA(c, cudaMemsetAsync(sa.turn, 0, ((size_t)sa.T * (kRounds + 1) + 2) * sizeof(int), c->stream));
+        kernel<<<grid, K::NT, smem, c->stream>>>(sa);
+        c->chain_launched = true;
+        return NB_OK;
+    }
     auto kernel = nb_gravity_sym_kernel<S, K::NI, K::NT, K::MINB, K::UNR>;
     static bool configured = false;                   // the kernel's shared memory is dynamic (112 KB at S = 4096)
     if (!configured) {
-        NB_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSymSmemPerElem * S));
+        NB_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
         configured = true;
     }
-    kernel<<<grid, K::NT, kSymSmemPerElem * S, c->stream>>>(sa);
+    kernel<<<grid, K::NT, smem, c->stream>>>(sa);
     return NB_OK;
 }
 
 template <int S>
-const char* sym_name()
+const char* sym_name(bool chain)
 {
     using K = SymShape<S>;
-    static char buf[64];
-    std::snprintf(buf, sizeof(buf), "nb_gravity_sym_kernel<%d,%d,%d,%d,%d>", S, K::NI, K::NT, K::MINB, K::UNR);
-    return buf;
+    static char buf[2][72];
+    std::snprintf(buf[chain], sizeof(buf[chain]), "nb_gravity_sym_%skernel<%d,%d,%d,%d,%d>", chain ? "chain_" : "", S, K::NI, K::NT,
+                  K::MINB, K::UNR);
+    return buf[chain];
 }
 
 // Row a2: partial gravitational accelerations -> part[0..ngrav-1][n]
@@ -282,7 +307,7 @@ int launch_gravity(nb_ctx* c)
 {
     if (c->plan.sym_S) {
         SymArgs sa;
-        sa.posm = c->posm; sa.part = c->part(); sa.n = (int)c->n; sa.T = c->plan.T;
+        sa.posm = c->posm; sa.part = c->part(); sa.acc64 = nullptr; sa.turn = nullptr; sa.n = (int)c->n; sa.T = c->plan.T;
         sa.G = c->prm.G; sa.eps = c->prm.eps;
         const long long T = c->plan.T;
         const int grid = (int)(T * (T + 1) / 2);
@@ -409,6 +434,7 @@ int launch_update(nb_ctx* c, const float4* src, int nsrc, float4* acc_out, float
                   int advance, float vscale = 1.f)
 {
     UpdateArgs u;
+    u.acc64 = (src == c->part() && c->plan.sym_S && c->plan.chain) ? c->at<double>(c->lay.off_acc64) : nullptr;
     u.src = src; u.acc_out = acc_out; u.posm = c->posm; u.vel = c->vel; u.dev = c->dev();
     u.n = (int)c->n; u.nsrc = nsrc; u.kick_h = kick_h; u.drift_dt = drift_dt; u.advance = advance; u.vscale = vscale;
     const int grid = (int)((c->n + 255) / 256);
@@ -441,6 +467,21 @@ int launch_fused(nb_ctx* c, int nforce, int open, int close_mode, float4* acc_ou
     NB_CUDA(c, cudaLaunchCooperativeKernel((const void*)nb_fused_step_kernel, dim3((unsigned)blocks), dim3(kThreads), args, 0,
                                            c->stream));
     c->launches++;
+    return NB_OK;
+}
+
+// Chain mode: a turn that never came (it cannot, by the ticket order -- this is the safety net that keeps a bug from
+// hanging the GPU) raises a flag on the device; the synchronising entry points report it.
+int chain_flag_check(nb_ctx* c)
+{
+    if (!c->have_state || !c->plan.sym_S || !c->plan.chain || !c->chain_launched) return NB_OK;
+    const int S = c->plan.sym_S;
+    const int rounds = S == 1024 ? 1 : (S == 2048 ? 2 : 4);
+    int flag = 0;
+    NB_CUDA(c, cudaMemcpyAsync(&flag, c->at<int>(c->lay.off_turn) + (size_t)c->plan.T * (rounds + 1) + 1, sizeof(int),
+                               cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (flag) { c->last_cuda = (int)cudaErrorLaunchTimeout; return NB_ECUDA; }
     return NB_OK;
 }
 
@@ -541,6 +582,7 @@ int nb_set_state(nb_ctx* c, int64_t n, float* posm, float* vel, const int32_t* s
     if (workspace_bytes < c->lay.total) return NB_ENOMEM;
     c->have_state = false;
     c->have_acc = false;
+    c->chain_launched = false;
     c->ws = static_cast<char*>(workspace);
 
     DevState h;
@@ -715,6 +757,7 @@ int nb_get_step(nb_ctx* c, int64_t* step, float* R)
     DevState h;
     NB_CUDA(c, cudaMemcpyAsync(&h, c->dev(), sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (const int rc = chain_flag_check(c)) return rc;
     if (step) *step = h.step;
     if (R) { R[0] = h.R[0]; R[1] = h.R[1]; }
     return NB_OK;
@@ -735,6 +778,8 @@ int nb_energy(nb_ctx* c, double* out)
     if (!c || !out) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
     int rc = ensure_acc(c);
+    if (rc) return rc;
+    rc = chain_flag_check(c);
     if (rc) return rc;
     const int n = (int)c->n;
     double* red_m = c->red();
@@ -800,7 +845,7 @@ int nb_download_state(nb_ctx* c, float* host_posm, float* host_vel, float* host_
     if (host_posm) NB_CUDA(c, cudaMemcpyAsync(host_posm, c->posm, bytes, cudaMemcpyDeviceToHost, c->stream));
     if (host_vel) NB_CUDA(c, cudaMemcpyAsync(host_vel, c->vel, bytes, cudaMemcpyDeviceToHost, c->stream));
     NB_CUDA(c, cudaStreamSynchronize(c->stream));
-    return NB_OK;
+    return chain_flag_check(c);
 }
 
 int nb_get_launch_info(nb_ctx* c, int32_t* out4)
@@ -825,7 +870,7 @@ int nb_set_force_path(nb_ctx* c, int path)
     if (!c || path < kPathAuto || path > kPathSymmetric) return NB_EINVAL;
     if (c->have_state) {
         const Plan p = make_plan(c->n, c->num_sms, path);
-        const int64_t ngrav = p.sym_S ? p.T : p.nsplit;
+        const int64_t ngrav = p.sym_S ? (p.chain ? 0 : p.T) : p.nsplit;
         if ((ngrav + c->ncontact()) * c->n > partial_elems_bound(c->n_max)) return NB_ENOMEM;
         c->plan = p;
     }
@@ -836,11 +881,11 @@ int nb_set_force_path(nb_ctx* c, int path)
 const char* nb_force_kernel_name(nb_ctx* c)
 {
     if (!c || !c->have_state) return "";
-    if (c->plan.sym_S == 256) return sym_name<256>();
-    if (c->plan.sym_S == 512) return sym_name<512>();
-    if (c->plan.sym_S == 1024) return sym_name<1024>();
-    if (c->plan.sym_S == 2048) return sym_name<2048>();
-    if (c->plan.sym_S) return sym_name<4096>();
+    if (c->plan.sym_S == 256) return sym_name<256>(c->plan.chain);
+    if (c->plan.sym_S == 512) return sym_name<512>(c->plan.chain);
+    if (c->plan.sym_S == 1024) return sym_name<1024>(c->plan.chain);
+    if (c->plan.sym_S == 2048) return sym_name<2048>(c->plan.chain);
+    if (c->plan.sym_S) return sym_name<4096>(c->plan.chain);
     return c->plan.TJ == 256 ? "nb_gravity_kernel<2,256>" : "nb_gravity_kernel<2,128>";
 }
 

@@ -59,7 +59,7 @@ nb_fused_step_kernel(const __grid_constant__ FusedArgs f)
     // four are dealt round-robin to the CTAs so that all of them have work.
     auto update = [&](const float4* src, int nsrc, float4* out0, float4* out1, float kick_h, float drift_dt) {
         UpdateArgs u;
-        u.src = src; u.acc_out = out0; u.posm = f.posm; u.vel = f.vel; u.dev = f.dev;
+        u.acc64 = nullptr; u.src = src; u.acc_out = out0; u.posm = f.posm; u.vel = f.vel; u.dev = f.dev;
         u.n = f.n; u.nsrc = nsrc; u.kick_h = kick_h; u.drift_dt = drift_dt; u.vscale = 1.f; u.advance = 0;
         const int q = threadIdx.x & 3, g = threadIdx.x >> 2;                 // 32 groups of four lanes per CTA
         for (int i0 = 0; i0 < f.n; i0 += gridDim.x * (kThreads / 4)) {       // uniform trip count: the shuffles need all lanes

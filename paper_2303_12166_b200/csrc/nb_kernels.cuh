@@ -382,10 +382,47 @@ nb_gravity_kernel(const __grid_constant__ GravArgs a)
 // (d and r^2 of all, then all MUFU.RSQ, ...), which keeps the MUFU of all of them in flight together.
 struct SymArgs {
     const float4* __restrict__ posm;   // [n] x,y,z,m
-    float4* __restrict__ part;         // [T][n]
+    float4* __restrict__ part;         // [T][n]   (slab mode)
+    double* __restrict__ acc64;        // [6][n]   (chain mode) a_i side x,y,z then reaction side x,y,z
+    int* __restrict__ turn;            // (chain mode) turnA[T rounds], turnR[T], ticket, error flag -- zero at launch
     int n, T;                          // T = ceil(n / S) super-tiles
     float G, eps;
 };
+
+// Chain mode (n >= 98,304): instead of T slabs of partial sums -- 1.1 GB at N = 262,144, 5 GB at 1,048,576 --
+// the CTAs add their results straight into ONE pair of fp64 accumulators per element, each super-tile's
+// contributions in a fixed order enforced by a turn counter per tile: bitwise reproducible, no atomics on data.
+// A CTA takes a ticket when it STARTS (so every lower ticket belongs to a CTA that is resident or done -- the
+// forward-progress argument of a decoupled look-back scan) and the tickets walk the pairs of super-tiles in
+// DIAGONAL-MAJOR order (d = B - A = 0, 1, 2, ...): the a_i side of (A, B) goes to tile A at turn d, after
+// (A, B-1); its reaction goes to tile B at turn d-1, after (A+1, B) -- both predecessors lie on the previous
+// diagonal, i.e. hold lower tickets, taken ~T tickets (a whole wave of CTAs) earlier: a CTA finds that its turn
+// has come when it gets there, the waits cost nothing, and no CTA ever waits for a higher ticket.
+__device__ __forceinline__ int ld_acquire_gpu(const int* p) {
+    int v; asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory"); return v;
+}
+__device__ __forceinline__ void st_release_gpu(int* p, int v) {
+    asm volatile("st.release.gpu.global.s32 [%0], %1;" :: "l"(p), "r"(v) : "memory");
+}
+constexpr int kChainSpinLimit = 1 << 22;     // x 100 ns: ~0.4 s, then the error flag is raised and the CTA goes on
+
+// Block-wide: wait until *turn == want (thread 0 polls; a lost turn raises *err instead of hanging the GPU).
+__device__ __forceinline__ void chain_wait(int* turn, int want, int* err) {
+    if (threadIdx.x == 0) {
+        int spins = 0;
+        while (ld_acquire_gpu(turn) != want) {
+            __nanosleep(100);
+            if (++spins > kChainSpinLimit) { atomicExch(err, 1); break; }
+        }
+    }
+    __syncthreads();
+}
+// Block-wide: publish the block's accumulator updates and pass the turn on.  The barrier orders the other
+// threads' stores before thread 0's release, which is cumulative: no fence per thread.
+__device__ __forceinline__ void chain_release(int* turn, int next) {
+    __syncthreads();
+    if (threadIdx.x == 0) st_release_gpu(turn, next);
+}
 
 constexpr int kSymSmemPerElem = 28;    // dynamic shared memory of the symmetric kernel: (16 + 3*4) bytes x S
 
@@ -454,7 +491,7 @@ __device__ __forceinline__ void sym_step(const f32x2 X, const f32x2 Y, const f32
     }
 }
 
-template <int S, int NI, int NT, int UNR, bool UNI, bool SYM>
+template <int S, int NI, int NT, int UNR, bool UNI, bool SYM, bool CHAIN = false>
 __device__ __forceinline__ void sym_sweep(const SymArgs& a, const int A, const int B,
                                            const float2* __restrict__ X2, const float2* __restrict__ Y2,
                                            const float2* __restrict__ Z2, const float2* __restrict__ M2,
@@ -513,24 +550,48 @@ __device__ __forceinline__ void sym_sweep(const SymArgs& a, const int A, const i
                 __syncthreads();                     // fixed order of the shared-memory sums
             }
         }
+        // chain mode: the turn counters of tile A are per ROUND (sub-tile of IPR elements), so that a pair of
+        // super-tiles with several rounds hands each of them on as soon as it is done
+        int* turnA = a.turn + (A * (S / IPR) + r);
+        if (CHAIN) chain_wait(turnA, B - A, a.turn + a.T * (S / IPR + 1) + 1);        // after round r of (A, B-1)
+        double vx[NI], vy[NI], vz[NI];
 #pragma unroll
         for (int i = 0; i < NI; ++i) {
-            const int e = ibase + i * 32;
             float xl, xh, yl, yh, zl, zh;
             unpk2(ax[i], xl, xh); unpk2(ay[i], yl, yh); unpk2(az[i], zl, zh);
-            if (e < a.n) out[e] = make_float4((float)(scale_i * ((double)xl + (double)xh)),
-                                              (float)(scale_i * ((double)yl + (double)yh)),
-                                              (float)(scale_i * ((double)zl + (double)zh)), 0.f);
+            vx[i] = scale_i * ((double)xl + (double)xh); vy[i] = scale_i * ((double)yl + (double)yh);
+            vz[i] = scale_i * ((double)zl + (double)zh);
+        }
+        if (CHAIN) {
+            const size_t n = (size_t)a.n;
+            if (A != B) {                            // all loads in flight together, then all stores (turn 0 stores only)
+#pragma unroll
+                for (int i = 0; i < NI; ++i) {
+                    const int e = ibase + i * 32;
+                    if (e < a.n) { vx[i] += __ldcg(a.acc64 + e); vy[i] += __ldcg(a.acc64 + n + e); vz[i] += __ldcg(a.acc64 + 2 * n + e); }
+                }
+            }
+#pragma unroll
+            for (int i = 0; i < NI; ++i) {
+                const int e = ibase + i * 32;
+                if (e < a.n) { __stcg(a.acc64 + e, vx[i]); __stcg(a.acc64 + n + e, vy[i]); __stcg(a.acc64 + 2 * n + e, vz[i]); }
+            }
+            chain_release(turnA, B - A + 1);
+        } else {
+#pragma unroll
+            for (int i = 0; i < NI; ++i) {
+                const int e = ibase + i * 32;
+                if (e < a.n) out[e] = make_float4((float)vx[i], (float)vy[i], (float)vz[i], 0.f);
+            }
         }
     }
 }
 
-template <int S, int NI, int NT, int MINB, int UNR>
-__global__ void __launch_bounds__(NT, MINB)
-nb_gravity_sym_kernel(const __grid_constant__ SymArgs a)
+// One pair of super-tiles (A <= B): stage B, sweep A's elements over it, write or chain the two results.
+template <int S, int NI, int NT, int UNR, bool CHAIN>
+__device__ __forceinline__ void sym_tile_pair(const SymArgs& a, const int A, const int B, float4* sym_smem)
 {
-    extern __shared__ float4 sym_smem[];             // 7 arrays of S/2 float2 = 28 S bytes
-    float2* __restrict__ X2 = reinterpret_cast<float2*>(sym_smem);
+    float2* __restrict__ X2 = reinterpret_cast<float2*>(sym_smem);      // 7 arrays of S/2 float2 = 28 S bytes
     float2* __restrict__ Y2 = X2 + S / 2;
     float2* __restrict__ Z2 = Y2 + S / 2;
     float2* __restrict__ M2 = Z2 + S / 2;
@@ -538,21 +599,6 @@ nb_gravity_sym_kernel(const __grid_constant__ SymArgs a)
     float2* __restrict__ JY = JX + S / 2;
     float2* __restrict__ JZ = JY + S / 2;
     const int tid = threadIdx.x;
-
-    int A, B;
-    {
-        const long long T = a.T, M = T * (T - 1) / 2, b = blockIdx.x;
-        if (b >= M) { A = B = (int)(b - M); }
-        else {
-            const double t2 = 2.0 * (double)T - 1.0;
-            long long r = (long long)((t2 - sqrt(t2 * t2 - 8.0 * (double)b)) * 0.5);
-            if (r < 0) r = 0;
-            while (r > 0 && r * (2 * T - r - 1) / 2 > b) --r;
-            while ((r + 1) * (2 * T - r - 2) / 2 <= b) ++r;
-            A = (int)r;
-            B = (int)(b - r * (2 * T - r - 1) / 2 + r + 1);
-        }
-    }
 
     // stage super-tile B as packed pairs: pair p of tile t holds elements 64 t + p and 64 t + 32 + p
     const float mB = a.posm[min(B * S, a.n - 1)].w, mA = a.posm[min(A * S, a.n - 1)].w;
@@ -571,25 +617,104 @@ nb_gravity_sym_kernel(const __grid_constant__ SymArgs a)
     const int uni = __syncthreads_and(u ? 1 : 0);
 
     if (A == B) {
-        if (uni) sym_sweep<S, NI, NT, UNR, true, false>(a, A, B, X2, Y2, Z2, M2, JX, JY, JZ, (double)(a.G * mB));
-        else     sym_sweep<S, NI, NT, UNR, false, false>(a, A, B, X2, Y2, Z2, M2, JX, JY, JZ, 1.0);
+        if (uni) sym_sweep<S, NI, NT, UNR, true, false, CHAIN>(a, A, B, X2, Y2, Z2, M2, JX, JY, JZ, (double)(a.G * mB));
+        else     sym_sweep<S, NI, NT, UNR, false, false, CHAIN>(a, A, B, X2, Y2, Z2, M2, JX, JY, JZ, 1.0);
+        if (CHAIN && A == 0) {                       // tile 0 receives no reaction at all: its sums are zero
+            for (int e = tid; e < S && e < a.n; e += NT) {
+                double* px = a.acc64 + 3 * (size_t)a.n + e;
+                __stcg(px, 0.0); __stcg(px + a.n, 0.0); __stcg(px + 2 * (size_t)a.n, 0.0);
+            }
+        }
         return;
     }
-    if (uni) sym_sweep<S, NI, NT, UNR, true, true>(a, A, B, X2, Y2, Z2, M2, JX, JY, JZ, (double)(a.G * mB));
-    else     sym_sweep<S, NI, NT, UNR, false, true>(a, A, B, X2, Y2, Z2, M2, JX, JY, JZ, 1.0);
+    if (uni) sym_sweep<S, NI, NT, UNR, true, true, CHAIN>(a, A, B, X2, Y2, Z2, M2, JX, JY, JZ, (double)(a.G * mB));
+    else     sym_sweep<S, NI, NT, UNR, false, true, CHAIN>(a, A, B, X2, Y2, Z2, M2, JX, JY, JZ, 1.0);
 
     const double scale_j = uni ? -(double)(a.G * mA) : -1.0;
     float4* __restrict__ outj = a.part + (size_t)A * a.n;
-    for (int p = tid; p < S / 2; p += NT) {
-        const int e0 = (p >> 5) * 64 + (p & 31), e1 = e0 + 32;
-        const float2 x = JX[p], y = JY[p], z = JZ[p];
-        if (B * S + e0 < a.n)
-            outj[B * S + e0] = make_float4((float)(scale_j * (double)x.x), (float)(scale_j * (double)y.x),
-                                           (float)(scale_j * (double)z.x), 0.f);
-        if (B * S + e1 < a.n)
-            outj[B * S + e1] = make_float4((float)(scale_j * (double)x.y), (float)(scale_j * (double)y.y),
-                                           (float)(scale_j * (double)z.y), 0.f);
+    constexpr int RNDS = S / (NT / 32 * 32 * NI);            // rounds per super-tile: turn counters [T RNDS] a_i side, [T] reaction
+    int* turnR = a.turn + a.T * RNDS + B;
+    if (CHAIN) chain_wait(turnR, B - A - 1, a.turn + a.T * (RNDS + 1) + 1);        // tile B's turn d - 1: after (A+1, B)
+    constexpr int PER = (S / 2 + NT - 1) / NT;               // packed pairs per thread
+    double v[PER][6];
+    const size_t n = (size_t)a.n;
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        const int p = tid + k * NT;
+        const float2 x = p < S / 2 ? JX[p] : make_float2(0.f, 0.f), y = p < S / 2 ? JY[p] : x, z = p < S / 2 ? JZ[p] : x;
+        v[k][0] = scale_j * (double)x.x; v[k][1] = scale_j * (double)y.x; v[k][2] = scale_j * (double)z.x;
+        v[k][3] = scale_j * (double)x.y; v[k][4] = scale_j * (double)y.y; v[k][5] = scale_j * (double)z.y;
     }
+    if (CHAIN && B - A > 1) {                                // all loads in flight together (turn 0 stores only)
+#pragma unroll
+        for (int k = 0; k < PER; ++k) {
+            const int p = tid + k * NT;
+            const int e0 = B * S + (p >> 5) * 64 + (p & 31), e1 = e0 + 32;
+            double* q = a.acc64 + 3 * n;
+            if (p < S / 2 && e0 < a.n) { v[k][0] += __ldcg(q + e0); v[k][1] += __ldcg(q + n + e0); v[k][2] += __ldcg(q + 2 * n + e0); }
+            if (p < S / 2 && e1 < a.n) { v[k][3] += __ldcg(q + e1); v[k][4] += __ldcg(q + n + e1); v[k][5] += __ldcg(q + 2 * n + e1); }
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < PER; ++k) {
+        const int p = tid + k * NT;
+        const int e0 = B * S + (p >> 5) * 64 + (p & 31), e1 = e0 + 32;
+        if (p >= S / 2) continue;
+        if (CHAIN) {
+            double* q = a.acc64 + 3 * n;
+            if (e0 < a.n) { __stcg(q + e0, v[k][0]); __stcg(q + n + e0, v[k][1]); __stcg(q + 2 * n + e0, v[k][2]); }
+            if (e1 < a.n) { __stcg(q + e1, v[k][3]); __stcg(q + n + e1, v[k][4]); __stcg(q + 2 * n + e1, v[k][5]); }
+        } else {
+            if (e0 < a.n) outj[e0] = make_float4((float)v[k][0], (float)v[k][1], (float)v[k][2], 0.f);
+            if (e1 < a.n) outj[e1] = make_float4((float)v[k][3], (float)v[k][4], (float)v[k][5], 0.f);
+        }
+    }
+    if (CHAIN) chain_release(turnR, B - A);
+}
+
+
+template <int S, int NI, int NT, int MINB, int UNR>
+__global__ void __launch_bounds__(NT, MINB)
+nb_gravity_sym_kernel(const __grid_constant__ SymArgs a)
+{
+    extern __shared__ float4 sym_smem[];
+    int A, B;
+    {
+        const long long T = a.T, M = T * (T - 1) / 2, b = blockIdx.x;
+        if (b >= M) { A = B = (int)(b - M); }
+        else {
+            const double t2 = 2.0 * (double)T - 1.0;
+            long long r = (long long)((t2 - sqrt(t2 * t2 - 8.0 * (double)b)) * 0.5);
+            if (r < 0) r = 0;
+            while (r > 0 && r * (2 * T - r - 1) / 2 > b) --r;
+            while ((r + 1) * (2 * T - r - 2) / 2 <= b) ++r;
+            A = (int)r;
+            B = (int)(b - r * (2 * T - r - 1) / 2 + r + 1);
+        }
+    }
+    sym_tile_pair<S, NI, NT, UNR, false>(a, A, B, sym_smem);
+}
+
+// Chain mode: every CTA takes a ticket when it starts and works on that pair of super-tiles, diagonal-major.
+template <int S, int NI, int NT, int MINB, int UNR>
+__global__ void __launch_bounds__(NT, MINB)
+nb_gravity_sym_chain_kernel(const __grid_constant__ SymArgs a)
+{
+    extern __shared__ float4 sym_smem[];
+    __shared__ int s_ticket;
+    constexpr int RNDS = S / (NT / 32 * 32 * NI);
+    if (threadIdx.x == 0) s_ticket = atomicAdd(a.turn + a.T * (RNDS + 1), 1);
+    __syncthreads();
+    const long long T = a.T, t = s_ticket;
+    // diagonal d holds T - d pairs; c(d) = d T - d (d - 1) / 2 pairs lie on the diagonals before it
+    const double t2 = 2.0 * (double)T + 1.0;
+    long long d = (long long)((t2 - sqrt(t2 * t2 - 8.0 * (double)t)) * 0.5);
+    if (d < 0) d = 0;
+    if (d > T - 1) d = T - 1;
+    while (d > 0 && d * T - d * (d - 1) / 2 > t) --d;
+    while (d < T - 1 && (d + 1) * T - (d + 1) * d / 2 <= t) ++d;
+    const int A = (int)(t - (d * T - d * (d - 1) / 2));
+    sym_tile_pair<S, NI, NT, UNR, true>(a, A, A + (int)d, sym_smem);
 }
 
 // ---------------------------------------------------------------------------
@@ -875,6 +1000,7 @@ nb_contact_chunk_kernel(const __grid_constant__ ContactArgs a, const int cg, con
 //   v_i += kick_h * a_i ;  x_i += drift_dt * v_i        (either may be 0)
 //   if advance: step += 1, R_s = ramp(step)             (expanding-star rule)
 struct UpdateArgs {
+    const double* acc64;               // chain mode: [6][n] fp64 sums (a_i side x,y,z; reaction x,y,z), else nullptr
     const float4* src;                 // [nsrc][n]
     float4* acc_out;                   // may be null; may alias src when nsrc == 1
     float4* posm;
@@ -930,6 +1056,11 @@ __device__ __forceinline__ void apply_update(const UpdateArgs& u, const int i, c
 __device__ __forceinline__ float4 update_element(const UpdateArgs& u, const int i, float4& p, float4& v)
 {
     double sx = 0.0, sy = 0.0, sz = 0.0;
+    if (u.acc64) {
+        const size_t n = (size_t)u.n;
+        const double* q = u.acc64 + i;
+        sx = q[0] + q[3 * n]; sy = q[n] + q[4 * n]; sz = q[2 * n] + q[5 * n];
+    }
 #pragma unroll 8
     for (int q = 0; q < u.nsrc; ++q) {
         const float4 t = u.src[(size_t)q * u.n + i];

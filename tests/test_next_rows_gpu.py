@@ -284,7 +284,7 @@ def test_bench_line_has_the_contract_keys(nb):
     # frac is what the ALUs executed (< 1); the algorithmic 21-flop figure sits beside it and may reach 1
     assert r["bound"] == "alu" and r["unit"] == "TFLOP/s" and 0.3 < r["frac"] < 0.9 and r["frac"] < r["frac_algorithmic"] < 1.2
     assert 0.3 < r["fma_pipe_frac"] < 1.0 and 0.3 < r["xu_pipe_frac"] < 1.0
-    assert r["kernel"].startswith("nb_gravity_sym_kernel<1024") and 0.9 < r["kernel_share_of_step"] <= 1.0
+    assert r["kernel"].startswith("nb_gravity_sym_chain_kernel<1024") and 0.9 < r["kernel_share_of_step"] <= 1.0
     assert abs(r["achieved"] / r["peak"] - r["frac"]) < 1e-9
     assert r["traffic"] is None or r["traffic"] > 0
     e = d["e2e"]

@@ -560,6 +560,33 @@ def test_full_length_runs_of_configs_3_and_4(nb, idx):
         assert t1["Mcross0"] >= t0["Mcross0"] and t1["M0"] == pytest.approx(t0["M0"], rel=1e-12)
 
 
+def test_chain_mode_is_bitwise_reproducible_and_agrees_with_the_one_sided_kernel(nb):
+    """n >= 98,304: the symmetric kernel adds into two fp64 sums per element in turn order instead of writing slabs.
+    Two runs give the same bits; the result agrees with the one-sided kernel to fp32 rounding; the workspace no
+    longer grows with the number of super-tiles."""
+    w = _ragged(70000, 31001, seed=51, eps=0.004)
+    p = params_f32(w.params)
+    outs = []
+    for _ in range(2):
+        s = _sim(nb, w, p)
+        assert nb.nb_force_kernel_name(s.ctx).startswith("nb_gravity_sym_chain_kernel<1024")
+        s.step(2)
+        a = s.compute_accel()
+        s.synchronize()
+        outs.append((s.posm.cpu().numpy().copy(), a.cpu().numpy().copy()))
+        assert nb.nb_get_step(s.ctx)[0] == 2                      # (also reads the chain's safety flag)
+        s.close()
+    assert np.array_equal(outs[0][0], outs[1][0]) and np.array_equal(outs[0][1], outs[1][1])
+    s = _sim(nb, w, p, force_path=nb.NB_PATH_ONE_SIDED)
+    s.step(2)
+    a1 = s.compute_accel().cpu().numpy().astype(np.float64)[:, :3]
+    s.close()
+    a2 = outs[0][1].astype(np.float64)[:, :3]
+    assert (np.linalg.norm(a1 - a2, axis=1) / np.linalg.norm(a1, axis=1)).max() < 1e-4      # 2 steps apart: switch decisions
+    assert np.median(np.linalg.norm(a1 - a2, axis=1) / np.linalg.norm(a1, axis=1)) < 1e-6
+    assert nb.nb_workspace_bytes(1 << 20) < (1 << 30) and nb.nb_workspace_bytes(1 << 23) < 3 * (1 << 30)
+
+
 @pytest.mark.parametrize("path", [1, 2])
 def test_results_are_bitwise_reproducible(nb, path):
     """Both gravity kernels sum in a fixed order (no atomics): two runs give the same bits."""
