@@ -146,8 +146,12 @@ Plan make_plan(int64_t n, int num_sms, int path)
 
 struct Layout {
     size_t off_dev, off_acc, off_part, off_red, off_ps, off_vs, off_gbox, off_sbox, off_cpart, off_cstate,
-        off_counters, off_bsum, off_bucket, off_slot, off_tmp, off_perm, off_acc64, off_turn, total;
+        off_counters, off_bsum, off_bucket, off_slot, off_tmp, off_perm, off_acc64, off_turn, off_epot, off_erep, total;
 };
+
+// Super-tile of nb_pot_pair_kernel for n elements (T <= 512 up to 2M elements), and its CTAs = fp64 partials.
+int pot_tile(int64_t n) { return n <= 524288 ? 1024 : (n <= 2097152 ? 4096 : 8192); }
+int64_t pot_pairs(int64_t n) { const int64_t T = (n + pot_tile(n) - 1) / pot_tile(n); return T * (T + 1) / 2; }
 
 // cell_cap(n1) + cell_cap(n - n1) < 4 n + 128 for every split of n <= n_max elements
 int64_t cell_counters_bound(int64_t n_max) { return 4 * n_max + 129; }
@@ -179,6 +183,8 @@ Layout make_layout(int64_t n_max)
     L.off_perm = o;     o += align_up((size_t)n_max * sizeof(uint32_t));
     L.off_acc64 = o;    o += align_up(n_max >= kChainMinN ? (size_t)n_max * 6 * sizeof(double) : 0);
     L.off_turn = o;     o += align_up(n_max >= kChainMinN ? ((size_t)(n_max / 1024 + 1) * 5 + 2) * sizeof(int) : 0);   // <= 4 rounds + 1 per tile
+    L.off_epot = o;     o += align_up((size_t)pot_pairs(n_max) * sizeof(double));
+    L.off_erep = o;     o += align_up(((size_t)n_max * 4 / kCcThreads + 1) * sizeof(double));
     L.total = o;
     return L;
 }
@@ -349,7 +355,7 @@ cudaError_t launch_after(bool pdl, void (*kernel)(P...), int grid, int block, cu
 }
 
 // Row a3: contact accelerations (Eqs. 5/6) of the pairs with r < R_i + R_j -> part[ngrav ...][n]
-int launch_contact_on(nb_ctx* c, cudaStream_t st)
+int launch_contact_on(nb_ctx* c, cudaStream_t st, double* epart = nullptr)
 {
     const int n = (int)c->n;
     ContactArgs ca;
@@ -366,7 +372,7 @@ int launch_contact_on(nb_ctx* c, cudaStream_t st)
         a.counters = c->at<int>(L.off_counters); a.bsum = c->at<int>(L.off_bsum);
         a.bucket = c->at<int>(L.off_bucket); a.slot = c->at<int>(L.off_slot); a.tmp = c->at<int>(L.off_tmp);
         a.perm = c->at<uint32_t>(L.off_perm); a.ps = c->ps(); a.vs = c->vs();
-        a.out = ca.out; a.law = ca;
+        a.out = ca.out; a.law = ca; a.epart = epart;
         a.n = n; a.n1 = c->n1;
         a.cap0 = (int)cell_cap(c->n1); a.cap1 = (int)cell_cap(c->n - c->n1); a.ncells = a.cap0 + a.cap1;
         a.lpe_log2 = c->n < kContactWideN ? 2 : 0;                  // lanes per element: 4 while the pass is latency-bound
@@ -382,11 +388,13 @@ int launch_contact_on(nb_ctx* c, cudaStream_t st)
         NB_CUDA(c, launch_after(pdl, nb_cell_scatter_kernel, (int)eb, kPassThreads, st, a));
         NB_CUDA(c, launch_after(pdl, nb_cell_rank_kernel, (int)eb, kPassThreads, st, a));
         cb = (((long long)n << a.lpe_log2) + kCcThreads - 1) / kCcThreads;
-        switch (a.lpe_log2) {
-            case 0: NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<0>, (int)cb, kCcThreads, st, a)); break;
-            case 1: NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<1>, (int)cb, kCcThreads, st, a)); break;
-            case 2: NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<2>, (int)cb, kCcThreads, st, a)); break;
-            default: NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<3>, (int)cb, kCcThreads, st, a)); break;
+        if (epart) {                                               // energy mode: U_rep partials instead of accelerations
+            if (a.lpe_log2) NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<2, true>, (int)cb, kCcThreads, st, a));
+            else            NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<0, true>, (int)cb, kCcThreads, st, a));
+        } else if (a.lpe_log2) {
+            NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<2>, (int)cb, kCcThreads, st, a));
+        } else {
+            NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<0>, (int)cb, kCcThreads, st, a));
         }
         c->launches += 7;
         NB_CUDA(c, cudaGetLastError());
@@ -784,22 +792,55 @@ int nb_energy(nb_ctx* c, double* out)
     const int n = (int)c->n;
     double* red_m = c->red();
     double* red_p = red_m + (size_t)kMomentBlocks * kMomentCols;
-    const int pot_blocks = (n + kThreads - 1) / kThreads;
     nb_moments_kernel<<<kMomentBlocks, 256, 0, c->stream>>>(c->posm, c->vel, c->acc(), n, red_m);
     c->launches++;
     NB_CUDA(c, cudaGetLastError());
-    PotArgs pa;
-    pa.posm = c->posm; pa.dev = c->dev(); pa.out = red_p; pa.n = n; pa.n1 = c->n1;
-    pa.G = c->prm.G; pa.eps = c->prm.eps; pa.gamma = c->prm.gamma;
-    nb_potential_kernel<<<pot_blocks, kThreads, 0, c->stream>>>(pa);
-    c->launches++;
-    NB_CUDA(c, cudaGetLastError());
+    size_t npot = 0, nrep = 0;                       // fp64 partials: U_grav (x 2 with U_rep interleaved for small n), U_rep
+    double *dpot = nullptr, *drep = nullptr;
+    const bool big = c->n >= kCellMinN;
+    if (big) {                                       // packed pair-of-super-tiles kernel + the cell list in energy mode
+        PotPairArgs pa;
+        pa.posm = c->posm; pa.out = dpot = c->at<double>(c->lay.off_epot);
+        pa.n = n; pa.G = c->prm.G; pa.eps = c->prm.eps;
+        const int S = pot_tile(c->n);
+        pa.T = (int)((c->n + S - 1) / S);
+        npot = (size_t)pot_pairs(c->n);
+        if (S == 1024)      nb_pot_pair_kernel<1024, 8, 128><<<(unsigned)npot, 128, 16 * 1024, c->stream>>>(pa);
+        else if (S == 4096) {
+            static bool cfg = false;
+            if (!cfg) { NB_CUDA(c, cudaFuncSetAttribute(nb_pot_pair_kernel<4096, 8, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 4096)); cfg = true; }
+            nb_pot_pair_kernel<4096, 8, 128><<<(unsigned)npot, 128, 16 * 4096, c->stream>>>(pa);
+        } else {
+            static bool cfg = false;
+            if (!cfg) { NB_CUDA(c, cudaFuncSetAttribute(nb_pot_pair_kernel<8192, 8, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 8192)); cfg = true; }
+            nb_pot_pair_kernel<8192, 8, 128><<<(unsigned)npot, 128, 16 * 8192, c->stream>>>(pa);
+        }
+        c->launches++;
+        NB_CUDA(c, cudaGetLastError());
+        if (c->contact_on()) {
+            drep = c->at<double>(c->lay.off_erep);
+            nrep = (size_t)((((long long)n << (c->n < kContactWideN ? 2 : 0)) + kCcThreads - 1) / kCcThreads);
+            rc = launch_contact_on(c, c->stream, drep);
+            if (rc) return rc;
+        }
+    } else {
+        const int pot_blocks = (n + kThreads - 1) / kThreads;
+        PotArgs pa;
+        pa.posm = c->posm; pa.dev = c->dev(); pa.out = dpot = red_p; pa.n = n; pa.n1 = c->n1;
+        pa.G = c->prm.G; pa.eps = c->prm.eps; pa.gamma = c->prm.gamma;
+        nb_potential_kernel<<<pot_blocks, kThreads, 0, c->stream>>>(pa);
+        c->launches++;
+        NB_CUDA(c, cudaGetLastError());
+        npot = (size_t)pot_blocks * 2;
+    }
 
-    const size_t nd = (size_t)kMomentBlocks * kMomentCols + (size_t)pot_blocks * 2;
-    double* h = new (std::nothrow) double[nd];
+    const size_t nm = (size_t)kMomentBlocks * kMomentCols;
+    double* h = new (std::nothrow) double[nm + npot + nrep];
     if (!h) return NB_ENOMEM;
     DevState hs;
-    cudaError_t e = cudaMemcpyAsync(h, red_m, nd * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+    cudaError_t e = cudaMemcpyAsync(h, red_m, nm * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h + nm, dpot, npot * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
+    if (e == cudaSuccess && nrep) e = cudaMemcpyAsync(h + nm + npot, drep, nrep * sizeof(double), cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(&hs, c->dev(), sizeof(hs), cudaMemcpyDeviceToHost, c->stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
     if (e != cudaSuccess) { delete[] h; c->last_cuda = (int)e; return NB_ECUDA; }
@@ -807,8 +848,13 @@ int nb_energy(nb_ctx* c, double* out)
     for (int b = 0; b < kMomentBlocks; ++b)
         for (int k = 0; k < kMomentCols; ++k) m[k] += h[(size_t)b * kMomentCols + k];
     double ug2 = 0.0, ur2 = 0.0;
-    const double* hp = h + (size_t)kMomentBlocks * kMomentCols;
-    for (int b = 0; b < pot_blocks; ++b) { ug2 += hp[2 * b]; ur2 += hp[2 * b + 1]; }
+    const double* hp = h + nm;
+    if (big) {
+        for (size_t b = 0; b < npot; ++b) ug2 += hp[b];
+        for (size_t b = 0; b < nrep; ++b) ur2 += hp[npot + b];
+    } else {
+        for (size_t b = 0; b < npot / 2; ++b) { ug2 += hp[2 * b]; ur2 += hp[2 * b + 1]; }
+    }
     delete[] h;
     out[0] = m[0];
     out[1] = -ug2;

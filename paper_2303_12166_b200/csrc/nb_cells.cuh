@@ -85,6 +85,7 @@ struct CellPassArgs {
     float4* __restrict__ ps;           // [n] x,y,z,R_star   (sorted by star, bucket, index)
     float4* __restrict__ vs;           // [n] vx,vy,vz,m
     float4* __restrict__ out;          // [n] contact acceleration, ORIGINAL index order
+    double* __restrict__ epart;        // energy mode (nb_energy): U_rep of the block's pairs, one fp64 partial per block
     ContactArgs law;                   // gamma, gamma_beta, v_dead, lens_mode
     int n, n1, cap0, cap1, ncells;     // cap_s: buckets of star s (0 or a power of two >= 64); ncells = cap0 + cap1
     int lpe_log2;                      // lanes per element of the contact phase: 1 << lpe_log2 <= 32
@@ -327,7 +328,9 @@ constexpr int kCcRound = 64;           // pairs a warp evaluates per round of th
 //      holds up 31 lanes with 4), evaluated in fp64 and handed back through shared memory; every lane adds
 //      up ITS pairs in the order it found them, and the lanes of an element are added by a fixed shuffle tree:
 //      the sums are bitwise reproducible.
-template <int LPL>
+// ENERGY = true (nb_energy, row a7): the same search, but every queued pair (k, j) with k < j in sorted order adds its
+// repulsion potential U_rep (reading A12) to one fp64 partial per block instead of a force to element k.
+template <int LPL, bool ENERGY = false>
 __global__ void __launch_bounds__(kCcThreads)
 nb_contact_cell_kernel(const __grid_constant__ CellPassArgs a)
 {
@@ -421,6 +424,7 @@ nb_contact_cell_kernel(const __grid_constant__ CellPassArgs a)
                         for (int h = 0; h < nh; ++h) {
                             const int jj = (int)hq[h][tid];
                             double fx, fy, fz;
+                            if (ENERGY) { if (k < jj) ax += contact_potential(a.law, pi, a.ps[jj]); continue; }
                             contact_pair(a.law, pi, vi, a.ps[jj], a.vs[jj], fx, fy, fz);
                             ax += fx * im; ay += fy * im; az += fz * im;
                         }
@@ -450,13 +454,15 @@ nb_contact_cell_kernel(const __grid_constant__ CellPassArgs a)
             const int ot = (tid & ~31) + lo;
             const int jj = (int)hq[p - pre[w][lo]][ot];
             const int ko = (int)((base + lo) >> LPL);
-            double fx, fy, fz;
-            contact_pair(a.law, a.ps[ko], a.vs[ko], a.ps[jj], a.vs[jj], fx, fy, fz);
+            double fx, fy = 0.0, fz = 0.0;
+            if (ENERGY) fx = ko < jj ? contact_potential(a.law, a.ps[ko], a.ps[jj]) : 0.0;
+            else contact_pair(a.law, a.ps[ko], a.vs[ko], a.ps[jj], a.vs[jj], fx, fy, fz);
             res[w][p - p0][0] = fx; res[w][p - p0][1] = fy; res[w][p - p0][2] = fz;
         }
         __syncwarp();
         const int b = max(mine0, p0), e = min(mine0 + nh, pe);
         for (int p = b; p < e; ++p) {
+            if (ENERGY) { ax += res[w][p - p0][0]; continue; }
             ax += res[w][p - p0][0] * im; ay += res[w][p - p0][1] * im; az += res[w][p - p0][2] * im;
         }
         __syncwarp();
@@ -466,6 +472,19 @@ nb_contact_cell_kernel(const __grid_constant__ CellPassArgs a)
         ax += __shfl_down_sync(0xffffffffu, ax, o);
         ay += __shfl_down_sync(0xffffffffu, ay, o);
         az += __shfl_down_sync(0xffffffffu, az, o);
+    }
+    if (ENERGY) {                                    // lane 0 of every element group holds the group's sum: add up the block's
+        __shared__ double esum[kCcThreads / 32];
+        double v = (valid && q == 0) ? ax : 0.0;
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) esum[w] = v;
+        __syncthreads();
+        if (tid == 0) {
+            double t = 0.0;
+            for (int i = 0; i < kCcThreads / 32; ++i) t += esum[i];
+            a.epart[blockIdx.x] = t;
+        }
+        return;
     }
     if (valid && q == 0) a.out[a.perm[k]] = make_float4((float)ax, (float)ay, (float)az, 0.f);
 }

@@ -876,6 +876,18 @@ __device__ __forceinline__ void contact_pair(const ContactArgs& a, const float4 
     fx = c * dx; fy = c * dy; fz = c * dz;
 }
 
+// Repulsion potential of one contact pair, reading A12: U_rep(r) = int_r^{2R} gamma pi V dr' = gamma pi h^3 (8R - h) / 48
+// with h = 2R - r, 2R = R_i + R_j (factored: no cancellation); 0 if the pair is not in contact.  fp64, as contact_pair().
+__device__ __forceinline__ double contact_potential(const ContactArgs& a, const float4 pi, const float4 pj)
+{
+    const double dx = (double)pj.x - (double)pi.x, dy = (double)pj.y - (double)pi.y, dz = (double)pj.z - (double)pi.z;
+    const double r2 = dx * dx + dy * dy + dz * dz;
+    const double D = (double)pi.w + (double)pj.w;
+    if (!(r2 < D * D) || r2 == 0.0) return 0.0;
+    const double h = D - sqrt(r2);
+    return (double)a.gamma * (3.14159265358979323846 / 48.0) * h * h * h * (4.0 * D - h);
+}
+
 // Squared gap between a point and an axis-aligned box (0 inside).
 __device__ __forceinline__ float point_gap2(const float4 p, const float4 lo, const float4 hi) {
     const float gx = fmaxf(0.f, fmaxf(lo.x - p.x, p.x - hi.x));
@@ -1197,6 +1209,131 @@ nb_potential_kernel(const __grid_constant__ PotArgs a)
     const double e1 = block_sum((double)a.G * (double)pi.w * phi, sh);
     const double e2 = block_sum(i < a.n ? urep : 0.0, sh);
     if (tid == 0) { a.out[2 * (size_t)blockIdx.x] = e1; a.out[2 * (size_t)blockIdx.x + 1] = e2; }
+}
+
+// Row a7 for n >= 8,192: U_grav = -sum_{i<j} G m_i m_j / (r + eps) over pairs of super-tiles (A <= B), one CTA each,
+// in the packed form of the symmetric gravity kernel: B staged in shared memory as packed pairs (broadcast LDS.64),
+// NI elements i of A per lane, per pair one MUFU.RSQ (r = r^2 y) and one MUFU.RCP (1/(r + eps)) -- the XU pipe bounds
+// it at the same N^2 MUFU as a force evaluation.  fp32 terms in chains of <= 128, flushed into fp64; one fp64
+// partial per CTA, summed on the host in CTA order.  A diagonal CTA (A == B) counts every ordered pair but the
+// self pair (masked by index) and halves the sum.  U_rep comes from the cell list (nb_cells.cuh, energy mode).
+struct PotPairArgs {
+    const float4* __restrict__ posm;   // [n] x,y,z,m
+    double* __restrict__ out;          // [T (T + 1) / 2]
+    int n, T;
+    float G, eps;
+};
+
+template <int NI, bool DIAG>
+__device__ __forceinline__ void pot_step(const f32x2 X, const f32x2 Y, const f32x2 Z, const f32x2 M, const int j0,
+                                         const float (&nxi)[NI], const float (&nyi)[NI], const float (&nzi)[NI],
+                                         const int (&ei)[NI], const f32x2 eps2, f32x2 (&acc)[NI])
+{
+    const f32x2 tiny2 = pk2(kTinyR2, kTinyR2);
+    f32x2 r2[NI], y[NI], sm[NI];
+#pragma unroll
+    for (int i = 0; i < NI; ++i) {
+        const f32x2 dx = add2(X, pk2(nxi[i], nxi[i])), dy = add2(Y, pk2(nyi[i], nyi[i])), dz = add2(Z, pk2(nzi[i], nzi[i]));
+        r2[i] = fma2(dx, dx, tiny2); r2[i] = fma2(dy, dy, r2[i]); r2[i] = fma2(dz, dz, r2[i]);
+    }
+#pragma unroll
+    for (int i = 0; i < NI; ++i) {
+        float a0, b0;
+        unpk2(r2[i], a0, b0);
+        y[i] = pk2(rsqrt_approx(a0), rsqrt_approx(b0));
+    }
+#pragma unroll
+    for (int i = 0; i < NI; ++i) sm[i] = fma2(r2[i], y[i], eps2);                 // r + eps
+#pragma unroll
+    for (int i = 0; i < NI; ++i) {
+        float a0, b0;
+        unpk2(sm[i], a0, b0);
+        f32x2 w = M;
+        if (DIAG) {                                  // the self pair does not count
+            float m0, m1;
+            unpk2(M, m0, m1);
+            w = pk2(j0 == ei[i] ? 0.f : m0, j0 + 1 == ei[i] ? 0.f : m1);
+        }
+        acc[i] = fma2(w, pk2(rcp_approx(a0), rcp_approx(b0)), acc[i]);            // m_j / (r + eps)
+    }
+}
+
+template <int S, int NI, int NT>
+__global__ void __launch_bounds__(NT, 3)
+nb_pot_pair_kernel(const __grid_constant__ PotPairArgs a)
+{
+    extern __shared__ float4 pot_smem[];             // X2, Y2, Z2, M2: 4 arrays of S/2 float2 = 16 S bytes
+    __shared__ double sh[NT / 32];
+    float2* __restrict__ X2 = reinterpret_cast<float2*>(pot_smem);
+    float2* __restrict__ Y2 = X2 + S / 2;
+    float2* __restrict__ Z2 = Y2 + S / 2;
+    float2* __restrict__ M2 = Z2 + S / 2;
+    constexpr int IPR = NT * NI;                     // elements i per round
+    static_assert(S % IPR == 0 && (S / 2) % 64 == 0, "whole rounds; whole flush intervals");
+    const int tid = threadIdx.x;
+    int A, B;
+    {
+        const long long T = a.T, Mo = T * (T - 1) / 2, b = blockIdx.x;
+        if (b >= Mo) { A = B = (int)(b - Mo); }
+        else {
+            const double t2 = 2.0 * (double)T - 1.0;
+            long long r = (long long)((t2 - sqrt(t2 * t2 - 8.0 * (double)b)) * 0.5);
+            if (r < 0) r = 0;
+            while (r > 0 && r * (2 * T - r - 1) / 2 > b) --r;
+            while ((r + 1) * (2 * T - r - 2) / 2 <= b) ++r;
+            A = (int)r;
+            B = (int)(b - r * (2 * T - r - 1) / 2 + r + 1);
+        }
+    }
+    for (int p = tid; p < S / 2; p += NT) {          // pair p holds elements 2 p and 2 p + 1 of B
+        const int e0 = B * S + 2 * p, e1 = e0 + 1;
+        float4 q0 = make_float4(kFarAway, kFarAway, kFarAway, 0.f), q1 = q0;
+        if (e0 < a.n) q0 = a.posm[e0];
+        if (e1 < a.n) q1 = a.posm[e1];
+        X2[p] = make_float2(q0.x, q1.x); Y2[p] = make_float2(q0.y, q1.y); Z2[p] = make_float2(q0.z, q1.z);
+        M2[p] = make_float2(q0.w, q1.w);
+    }
+    __syncthreads();
+    const f32x2 eps2 = pk2(a.eps, a.eps);
+    double total = 0.0;
+#pragma unroll 1
+    for (int r = 0; r < S / IPR; ++r) {
+        float nxi[NI], nyi[NI], nzi[NI], mi[NI];
+        int ei[NI];
+        double phi[NI];
+#pragma unroll
+        for (int i = 0; i < NI; ++i) {
+            ei[i] = A * S + r * IPR + i * NT + tid;
+            float4 q = make_float4(-kFarAway, -kFarAway, -kFarAway, 0.f);
+            if (ei[i] < a.n) q = a.posm[ei[i]];
+            nxi[i] = -q.x; nyi[i] = -q.y; nzi[i] = -q.z; mi[i] = q.w;
+            phi[i] = 0.0;
+        }
+#pragma unroll 1
+        for (int p0 = 0; p0 < S / 2; p0 += 64) {
+            f32x2 acc[NI];
+#pragma unroll
+            for (int i = 0; i < NI; ++i) acc[i] = pk2(0.f, 0.f);
+#pragma unroll 4
+            for (int p = p0; p < p0 + 64; ++p) {
+                const f32x2 X = *reinterpret_cast<const f32x2*>(X2 + p), Y = *reinterpret_cast<const f32x2*>(Y2 + p),
+                            Z = *reinterpret_cast<const f32x2*>(Z2 + p), M = *reinterpret_cast<const f32x2*>(M2 + p);
+                if (A == B) pot_step<NI, true>(X, Y, Z, M, B * S + 2 * p, nxi, nyi, nzi, ei, eps2, acc);
+                else        pot_step<NI, false>(X, Y, Z, M, 0, nxi, nyi, nzi, ei, eps2, acc);
+            }
+#pragma unroll
+            for (int i = 0; i < NI; ++i) {
+                float l, h;
+                unpk2(acc[i], l, h);
+                phi[i] += (double)l + (double)h;
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < NI; ++i) total += (double)mi[i] * phi[i];
+    }
+    total *= (A == B ? 0.5 : 1.0) * (double)a.G;
+    const double rsum = block_sum(total, sh);
+    if (tid == 0) a.out[blockIdx.x] = rsum;
 }
 
 // ---------------------------------------------------------------------------
