@@ -322,6 +322,10 @@ def run_own(args):
     from workloads.configs import CONFIGS, make_binary
     kw = dict(CONFIGS[args.config])
     kw["seed"] = kw["seed"] + rank
+    if args.scale != 1.0:                       # the same recipe at another size (crossover measurements; not a BASELINE config)
+        kw["n1"] = max(1, int(round(kw["n1"] * args.scale)))
+        kw["n2"] = max(1, int(round(kw["n2"] * args.scale)))
+        kw["name"] = f"{kw['name']}_x{args.scale:g}"
     w = make_binary(**kw)
     p = params_f32(w.params)
     n = w.n
@@ -516,6 +520,8 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, choices=[1, 2, 3, 4, 5], default=BENCH_CONFIG,
                     help="BASELINE config timed as the headline (default 4, the one the metric is quoted on)")
+    ap.add_argument("--scale", type=float, default=1.0,
+                    help="scale the element counts of --config (same recipe and seed): for crossover measurements only")
     ap.add_argument("--path", choices=["auto", "one-sided", "symmetric"], default="auto",
                     help="row-a2 kernel (nb_set_force_path); auto = the library's choice")
     ap.add_argument("--impl", choices=["own", "reference", "stub"], default="own")

@@ -68,10 +68,14 @@ def _check_accel(nb, w, p=None, rows=None, tol=ACC_TOL, contacts_per_element=5, 
     rel = np.maximum(err[ok] - dl[ok], 0.0) / an[ok]
     assert rel.max() <= tol, f"max rel err {rel.max():.3e} (kappa {kap[ok][np.argmax(rel)]:.1f}) launch {info}"
     assert (err[~ok] <= 1e-12).all()
+    namb = 0
     if p.get("gamma", 0.0) > 0:
-        _a6_population(w, p, sel, dl, cap=64 if contacts_per_element <= 5 else 1024)
+        _, namb = _a6_population(w, p, sel, dl, cap=64 if contacts_per_element <= 5 else 1024)
     else:
         assert (dl == 0).all()
+    # measured margin, for `pytest -s` (profiles/r2_parity_margins.md is made from these lines)
+    print(f"PARITY accel {w.name} n={w.n} rows={len(sel)} kernel={info} max_rel={rel.max():.3e} median_rel={np.median(rel):.3e} "
+          f"max_kappa={kap[ok].max():.1f} a6_pairs={namb}")
     return a_gpu, rel.max()
 
 
@@ -354,11 +358,21 @@ def _check_traj(nb, w, nsteps=10, chunks=None):
     assert np.allclose(R, o.radii(), rtol=0, atol=0), (R, o.radii())
     assert np.array_equal(x[:, 3], w.posm[:, 3].astype(np.float64))           # masses untouched
     perr = np.linalg.norm(x[:, :3] - o.x, axis=1).max() / w.meta["a"]
-    vscale = w.meta["omega"] * w.meta["a"]
-    verr = np.linalg.norm(v[:, :3] - o.v, axis=1).max() / vscale
+    verr = _check_velocities(v[:, :3], o.v, w)
     assert perr <= POS_TOL, perr
-    assert verr <= 1e-2, verr        # velocities carry dt * (contact-switch) differences; positions are the bar
+    print(f"PARITY traj {w.name} n={w.n} steps={nsteps} pos_err={perr:.3e} vel_err_max={verr:.3e}")
     return perr, verr
+
+
+def _check_velocities(v, v_or, w):
+    """north_star sets no bar for velocities; these are measured ones (profiles/r2_parity_margins.md: median 3e-6,
+    99.9 % quantile 3-6e-5 of omega a after 10 steps), with a factor ~10 of room.  Tight enough to catch a wrong
+    kick: a half kick too many or too few shifts EVERY element by dt |a| / 2 ~ 5e-3 omega a here.  The few elements
+    whose contact pair sits on the converging/diverging switch (A6) may differ by dt (1 - beta) gamma pi V / m."""
+    ve = np.linalg.norm(v - v_or, axis=1) / (w.meta["omega"] * w.meta["a"])
+    assert np.median(ve) <= 3e-5 and np.quantile(ve, 0.999) <= 5e-4, (np.median(ve), np.quantile(ve, 0.999))
+    assert ve.max() <= 5e-2, ve.max()
+    return float(ve.max())
 
 
 def test_ten_step_trajectory_config1(nb):
@@ -419,9 +433,8 @@ def test_ten_step_trajectory_full_size_against_stored_oracle(nb, idx):
     s.close()
     rows = gold[:, 0].astype(np.int64)
     perr = np.linalg.norm(x[rows, :3] - gold[:, 1:4], axis=1).max() / w.meta["a"]
-    verr = np.linalg.norm(v[rows, :3] - gold[:, 4:7], axis=1).max() / (w.meta["omega"] * w.meta["a"])
     assert perr <= POS_TOL, perr
-    assert verr <= 1e-2, verr
+    _check_velocities(v[rows, :3], gold[:, 4:7], w)
     assert np.isfinite(x).all() and np.isfinite(v).all() and e["step"] == 10
 
 
@@ -494,6 +507,7 @@ def test_energy_and_momenta_match_oracle(nb, kind):
     oe = o.energy()
     for k in ("KE", "Ug", "Urep", "E"):
         assert e[k] == pytest.approx(oe[k], rel=2e-6, abs=1e-12), (k, e[k], oe[k])
+    print(f"PARITY energy {kind} n={w.n} " + " ".join(f"{k}_rel={abs(e[k] - oe[k]) / max(abs(oe[k]), 1e-300):.2e}" for k in ("KE", "Ug", "Urep", "E")))
     pscale = float((w.posm[:, 3].astype(np.float64) * np.linalg.norm(v[:, :3].astype(np.float64), axis=1)).sum())
     assert np.abs(np.array(e["P"]) - oe["P"]).max() <= 1e-12 * pscale + 1e-15
     assert np.abs(np.array(e["L"]) - oe["L"]).max() <= 1e-12 * np.abs(oe["L"]).max() + 1e-12 * pscale
