@@ -202,6 +202,13 @@ int64_t nb_launch_count(nb_ctx* ctx);
 int nb_time_force_kernel(nb_ctx* ctx, int reps, float* ms_avg);
 int nb_time_contact_pass(nb_ctx* ctx, int reps, float* ms_avg);
 
+/* Measurement aid for row a3: one contact pass (which pairs are "in contact") in counting mode.
+ * HOST out2[0] = candidate pairs the search pre-tests (ordered: each element against the elements of the cells of
+ * its query), out2[1] = pairs that pass the fp32 pre-test and are evaluated in fp64 (about twice the number of
+ * unordered contacts).  n < 8192 (no cell list): out2[0] = n (n - 1), out2[1] = -1.  gamma == 0: zeros.
+ * The partial sums it writes touch no state.  Synchronises the stream. */
+int nb_contact_stats(nb_ctx* ctx, int64_t* out2);
+
 void nb_destroy(nb_ctx* ctx);
 const char* nb_strerror(int status);
 int nb_last_cuda_error(nb_ctx* ctx);

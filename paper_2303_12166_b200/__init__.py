@@ -22,7 +22,7 @@ EXPORTS = ("nb_create", "nb_workspace_bytes", "nb_set_state", "nb_compute_accel"
            "nb_energy", "nb_set_step", "nb_relax", "nb_transfer_diagnostics", "nb_splat", "nb_get_step", "nb_upload_state",
            "nb_download_state",
            "nb_get_launch_info", "nb_set_force_path", "nb_force_kernel_name", "nb_launch_count",
-           "nb_time_force_kernel", "nb_time_contact_pass", "nb_destroy", "nb_strerror",
+           "nb_time_force_kernel", "nb_time_contact_pass", "nb_contact_stats", "nb_destroy", "nb_strerror",
            "nb_last_cuda_error", "nb_roche_lobe_radius", "nb_l1_distance")
 
 
@@ -94,6 +94,8 @@ def lib() -> C.CDLL:
         L.nb_time_force_kernel.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
         L.nb_time_contact_pass.restype = C.c_int
         L.nb_time_contact_pass.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
+        L.nb_contact_stats.restype = C.c_int
+        L.nb_contact_stats.argtypes = [vp, C.POINTER(i64)]
         L.nb_destroy.restype = None
         L.nb_destroy.argtypes = [vp]
         L.nb_strerror.restype = C.c_char_p
@@ -241,6 +243,12 @@ def nb_time_contact_pass(ctx: int, reps: int) -> float:
     ms = C.c_float()
     _check(lib().nb_time_contact_pass(ctx, int(reps), C.byref(ms)), "nb_time_contact_pass", ctx)
     return float(ms.value)
+
+
+def nb_contact_stats(ctx: int) -> Dict[str, int]:
+    out = (C.c_int64 * 2)()
+    _check(lib().nb_contact_stats(ctx, out), "nb_contact_stats", ctx)
+    return dict(candidates=int(out[0]), queued=int(out[1]))
 
 
 def nb_destroy(ctx: int) -> None:

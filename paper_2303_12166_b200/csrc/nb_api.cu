@@ -355,7 +355,7 @@ cudaError_t launch_after(bool pdl, void (*kernel)(P...), int grid, int block, cu
 }
 
 // Row a3: contact accelerations (Eqs. 5/6) of the pairs with r < R_i + R_j -> part[ngrav ...][n]
-int launch_contact_on(nb_ctx* c, cudaStream_t st, double* epart = nullptr)
+int launch_contact_on(nb_ctx* c, cudaStream_t st, double* epart = nullptr, unsigned long long* stats = nullptr)
 {
     const int n = (int)c->n;
     ContactArgs ca;
@@ -372,7 +372,7 @@ int launch_contact_on(nb_ctx* c, cudaStream_t st, double* epart = nullptr)
         a.counters = c->at<int>(L.off_counters); a.bsum = c->at<int>(L.off_bsum);
         a.bucket = c->at<int>(L.off_bucket); a.slot = c->at<int>(L.off_slot); a.tmp = c->at<int>(L.off_tmp);
         a.perm = c->at<uint32_t>(L.off_perm); a.ps = c->ps(); a.vs = c->vs();
-        a.out = ca.out; a.law = ca; a.epart = epart;
+        a.out = ca.out; a.law = ca; a.epart = epart; a.stats = stats;
         a.n = n; a.n1 = c->n1;
         a.cap0 = (int)cell_cap(c->n1); a.cap1 = (int)cell_cap(c->n - c->n1); a.ncells = a.cap0 + a.cap1;
         a.lpe_log2 = c->n < kContactWideN ? 2 : 0;                  // lanes per element: 4 while the pass is latency-bound
@@ -391,6 +391,9 @@ int launch_contact_on(nb_ctx* c, cudaStream_t st, double* epart = nullptr)
         if (epart) {                                               // energy mode: U_rep partials instead of accelerations
             if (a.lpe_log2) NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<2, true>, (int)cb, kCcThreads, st, a));
             else            NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<0, true>, (int)cb, kCcThreads, st, a));
+        } else if (stats) {                                        // counting mode (nb_contact_stats)
+            if (a.lpe_log2) NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<2, false, true>, (int)cb, kCcThreads, st, a));
+            else            NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<0, false, true>, (int)cb, kCcThreads, st, a));
         } else if (a.lpe_log2) {
             NB_CUDA(c, launch_after(pdl, nb_contact_cell_kernel<2>, (int)cb, kCcThreads, st, a));
         } else {
@@ -962,6 +965,28 @@ int time_launches(nb_ctx* c, int reps, float* ms_avg, int (*launch)(nb_ctx*))
     return NB_OK;
 }
 }  // namespace
+
+int nb_contact_stats(nb_ctx* c, int64_t* out2)
+{
+    if (!c || !out2) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    out2[0] = out2[1] = 0;
+    if (!c->contact_on()) return NB_OK;
+    if (c->n < kCellMinN) {                                    // no cell list: every ordered pair is pre-tested
+        out2[0] = c->n * (c->n - 1);
+        out2[1] = -1;
+        return NB_OK;
+    }
+    unsigned long long* d = reinterpret_cast<unsigned long long*>(c->at<double>(c->lay.off_erep));
+    NB_CUDA(c, cudaMemsetAsync(d, 0, 2 * sizeof(unsigned long long), c->stream));
+    int rc = launch_contact_on(c, c->stream, nullptr, d);
+    if (rc) return rc;
+    unsigned long long h[2] = {0, 0};
+    NB_CUDA(c, cudaMemcpyAsync(h, d, sizeof(h), cudaMemcpyDeviceToHost, c->stream));
+    NB_CUDA(c, cudaStreamSynchronize(c->stream));
+    out2[0] = (int64_t)h[0]; out2[1] = (int64_t)h[1];
+    return NB_OK;
+}
 
 int nb_time_force_kernel(nb_ctx* c, int reps, float* ms_avg)
 {

@@ -86,6 +86,7 @@ struct CellPassArgs {
     float4* __restrict__ vs;           // [n] vx,vy,vz,m
     float4* __restrict__ out;          // [n] contact acceleration, ORIGINAL index order
     double* __restrict__ epart;        // energy mode (nb_energy): U_rep of the block's pairs, one fp64 partial per block
+    unsigned long long* __restrict__ stats;   // counting mode (nb_contact_stats): candidates pre-tested, pairs queued
     ContactArgs law;                   // gamma, gamma_beta, v_dead, lens_mode
     int n, n1, cap0, cap1, ncells;     // cap_s: buckets of star s (0 or a power of two >= 64); ncells = cap0 + cap1
     int lpe_log2;                      // lanes per element of the contact phase: 1 << lpe_log2 <= 32
@@ -330,7 +331,8 @@ constexpr int kCcRound = 64;           // pairs a warp evaluates per round of th
 //      the sums are bitwise reproducible.
 // ENERGY = true (nb_energy, row a7): the same search, but every queued pair (k, j) with k < j in sorted order adds its
 // repulsion potential U_rep (reading A12) to one fp64 partial per block instead of a force to element k.
-template <int LPL, bool ENERGY = false>
+// STATS = true (nb_contact_stats, a measurement aid): also counts the candidates it pre-tests and the pairs it queues.
+template <int LPL, bool ENERGY = false, bool STATS = false>
 __global__ void __launch_bounds__(kCcThreads)
 nb_contact_cell_kernel(const __grid_constant__ CellPassArgs a)
 {
@@ -356,6 +358,7 @@ nb_contact_cell_kernel(const __grid_constant__ CellPassArgs a)
     const bool valid = k < a.n;
     double ax = 0.0, ay = 0.0, az = 0.0;
     int nh = 0;
+    unsigned ncand = 0, nqueued = 0;
     float4 pi = make_float4(0.f, 0.f, 0.f, 0.f), vi = make_float4(0.f, 0.f, 0.f, 1.f);
     if (valid) {
         pi = a.ps[k]; vi = a.vs[k];
@@ -418,6 +421,7 @@ nb_contact_cell_kernel(const __grid_constant__ CellPassArgs a)
                     const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
                     hq[nh][tid] = (uint32_t)j;                       // kept only if it is a hit
                     nh += (r2 <= thr && j != k);
+                    if (STATS) { ++ncand; nqueued += (r2 <= thr && j != k); }
                     ++j;
                     if (nh == kCcQueue) {                            // queue full (dense overlaps): evaluate it here, in order
                         const double im = 1.0 / (double)vi.w;
@@ -433,6 +437,10 @@ nb_contact_cell_kernel(const __grid_constant__ CellPassArgs a)
                 }
             }
         }
+    }
+    if (STATS) {
+        for (int o = 16; o > 0; o >>= 1) { ncand += __shfl_xor_sync(0xffffffffu, ncand, o); nqueued += __shfl_xor_sync(0xffffffffu, nqueued, o); }
+        if (lane == 0) { atomicAdd(a.stats, (unsigned long long)ncand); atomicAdd(a.stats + 1, (unsigned long long)nqueued); }
     }
     // balanced evaluation of the warp's queued pairs
     __syncwarp();

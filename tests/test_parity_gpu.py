@@ -312,6 +312,29 @@ def test_contact_pass_with_far_outliers(nb):
     _check_accel(nb, w)
 
 
+@pytest.mark.parametrize("idx", [2, 3, 4, 5])
+def test_cell_list_tests_few_candidates_per_element(nb, idx):
+    """Row a3: the cell list pre-tests a few tens of candidates per element (the 27 cells of a query hold ~33 at the
+    configs' packing; the box search of round 1 tested ~960) and queues exactly the oracle's contact pairs plus the
+    handful the 1e-5 slack of the fp32 pre-test lets through."""
+    w = make_config(idx)
+    p = params_f32(w.params)
+    s = _sim(nb, w, p)
+    st = nb.nb_contact_stats(s.ctx)
+    a_before = s.compute_accel().clone()
+    assert nb.nb_contact_stats(s.ctx) == st                        # deterministic, and it touches no state
+    import torch
+    assert torch.equal(a_before, s.compute_accel())
+    s.close()
+    rows = _sample(w.n, 2048, 5 + idx)
+    cnt, _, _, _ = oracle.contact_list(w.posm, w.vel, w.star, p["R_start"], rows=rows, cap=8)
+    per_elem = st["candidates"] / w.n
+    print(f"PARITY contact_stats {w.name} n={w.n} candidates_per_element={per_elem:.1f} queued_per_element={st['queued'] / w.n:.2f} "
+          f"oracle_contacts_per_element={cnt.mean():.2f}")
+    assert per_elem <= 64.0
+    assert abs(st["queued"] / w.n - cnt.mean()) <= 4.0 * cnt.std() / np.sqrt(len(rows)) + 0.01
+
+
 def test_contact_pass_timing_entry_point(nb):
     w = make_config(2)
     p = params_f32(w.params)
