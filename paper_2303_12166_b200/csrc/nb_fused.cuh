@@ -42,11 +42,13 @@ struct FusedArgs {
     int close_mode;            // 0: the last update is the closing half kick; 1: it stores a(x) and moves nothing
 };
 
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, 4)
 nb_fused_step_kernel(const __grid_constant__ FusedArgs f)
 {
     __shared__ float4 sj[2][128];
     __shared__ uint32_t queue_s[kInlineQueue][kThreads];
+    __shared__ int pre_s[kThreads / 32][33];
+    __shared__ double res_s[kThreads / 32][kInlineRound * 3];
     cooperative_groups::grid_group grid = cooperative_groups::this_grid();
     const bool contact = f.law.gamma > 0.f;
 
@@ -98,7 +100,7 @@ nb_fused_step_kernel(const __grid_constant__ FusedArgs f)
         InlineContact ic;
         ic.law = &f.law; ic.vel = f.vel; ic.n1 = f.n1;
         ic.R0 = ramp_radius(Rs0, Re0, n_ramp, nstep); ic.R1 = ramp_radius(Rs1, Re1, n_ramp, nstep);
-        ic.q = &queue_s[0][threadIdx.x];
+        ic.q = &queue_s[0][threadIdx.x]; ic.pre = &pre_s[0][0]; ic.res = &res_s[0][0];
         for (int item = blockIdx.x; item < G; item += gridDim.x) {
             if (contact) gravity_block<2, 128, true>(f.grav, item, sj, ic);
             else         gravity_block<2, 128, false>(f.grav, item, sj);

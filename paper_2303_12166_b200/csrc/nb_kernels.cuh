@@ -116,7 +116,10 @@ struct InlineContact {
     int n1;
     float R0, R1;                      // element radius per star
     uint32_t* q;                       // the thread's queue: q[k * kThreads], k < kInlineQueue
+    int* pre;                          // [kThreads / 32][33]  scratch of the warp-balanced evaluation
+    double* res;                       // [kThreads / 32][kInlineRound][3]
 };
+constexpr int kInlineRound = 64;       // pairs a warp evaluates per round
 
 template <int H, bool UNI, bool CON>
 __device__ __forceinline__ void gravity_group(const float4* __restrict__ s,
@@ -257,6 +260,51 @@ __device__ __forceinline__ void gravity_block(const GravArgs& a, const int vb, f
         nq = 0;
     };
 
+    // The same at a point where the whole warp arrives together (the end of a tile): the warp's queued pairs are
+    // dealt evenly to its lanes -- a lane with 6 pairs no longer holds up 31 lanes with 1 -- evaluated, and handed
+    // back through shared memory; every lane adds up ITS pairs in the order it found them.
+    auto drain_warp = [&]() {
+        const int lane = tid & 31, wq = tid >> 5;
+        int inc = nq;
+        for (int o = 1; o < 32; o <<= 1) { const int t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+        const int total = __shfl_sync(0xffffffffu, inc, 31), mine0 = inc - nq;
+        int* pre = ic.pre + wq * 33;
+        double* res = ic.res + wq * (kInlineRound * 3);
+        pre[lane] = mine0;
+        if (lane == 31) pre[32] = total;
+        __syncwarp();
+        for (int p0 = 0; p0 < total; p0 += kInlineRound) {
+            const int pe = min(total, p0 + kInlineRound);
+            for (int p = p0 + lane; p < pe; p += 32) {
+                int lo = 0;                          // owner: the largest lane with pre[lane] <= p
+#pragma unroll
+                for (int s2 = 16; s2 > 0; s2 >>= 1) if (pre[lo + s2] <= p) lo += s2;
+                const uint32_t w = (q - lane)[(p - pre[lo]) * kThreads + lo];
+                const int j = (int)(w >> 4), i = ibase - lane + lo + (int)(w & 15u) * kThreads;
+                double fx = 0.0, fy = 0.0, fz = 0.0;
+                if (j < a.n && i < a.n && j != i) {
+                    const float4 xi = a.posm[i], wi = ic.vel[i], wj = ic.vel[j], xj = tile[j - tile_j0];
+                    contact_pair(*ic.law, make_float4(xi.x, xi.y, xi.z, star_radius(i, ic.n1, ic.R0, ic.R1)),
+                                 make_float4(wi.x, wi.y, wi.z, xi.w),
+                                 make_float4(xj.x, xj.y, xj.z, star_radius(j, ic.n1, ic.R0, ic.R1)), wj, fx, fy, fz);
+                    const double im = 1.0 / (double)xi.w;
+                    fx *= im; fy *= im; fz *= im;
+                }
+                res[(p - p0) * 3] = fx; res[(p - p0) * 3 + 1] = fy; res[(p - p0) * 3 + 2] = fz;
+            }
+            __syncwarp();
+            const int b = max(mine0, p0), e = min(mine0 + nq, pe);
+            for (int p = b; p < e; ++p) {
+                const int k = (int)(q[(p - mine0) * kThreads] & 15u);
+#pragma unroll
+                for (int kk = 0; kk < I; ++kk)
+                    if (kk == k) { accx[kk] += res[(p - p0) * 3]; accy[kk] += res[(p - p0) * 3 + 1]; accz[kk] += res[(p - p0) * 3 + 2]; }
+            }
+            __syncwarp();
+        }
+        nq = 0;
+    };
+
     float4 pre[LPT];
     bool my_uni = false;                             // this thread's share of the tile has one mass
     auto load_tile = [&](int t) {
@@ -316,7 +364,7 @@ __device__ __forceinline__ void gravity_block(const GravArgs& a, const int vb, f
                 if (CON && nq > kInlineQueue - 2 * kGroupJ * H) drain();
             }
         }
-        if (CON) drain();
+        if (CON) drain_warp();
 
         // flush the tile's fp32 sums into the fp64 accumulators (short fp32 chains)
 #pragma unroll
