@@ -51,7 +51,8 @@ constexpr int64_t kSymMinN = 10240;               // auto: symmetric kernel from
 constexpr int64_t kSym256MaxN = 32768;             // below this the super-tiles are 256 elements (CTAs of 2 warps)
 constexpr int64_t kSymMaxN = (int64_t)1 << 26;    // ... for every n the library takes
 constexpr int64_t kChainMinN = 98304;             // from here on (S >= 1,024) the symmetric kernel runs in chain mode: its T
-                                                  // slabs would be 1.1 GB at 262,144 elements and 5 GB at 1,048,576
+                                                  // slabs would be 1.1 GB at 262,144 elements and 5 GB at 1,048,576.  Not below:
+                                                  // with the short CTAs of S = 512 the turns do cost (65,536: 1.66 vs 1.20 ms)
 
 // Super-tile size of the symmetric kernel for n elements: its T = ceil(n/S) slabs of n float4
 // partial sums cost memory and one extra pass, so S grows with n.
