@@ -169,7 +169,7 @@ int nb_download_state(nb_ctx* ctx, float* host_posm, float* host_vel, float* hos
 int nb_get_launch_info(nb_ctx* ctx, int32_t* out4);
 
 /* Which kernel evaluates row a2 (Eq. 4, summed over all pairs).
- *   NB_PATH_AUTO (default): the symmetric kernel for n >= 10240, else the one-sided kernel (n < 8192:
+ *   NB_PATH_AUTO (default): the symmetric kernel for n >= 8192, else the one-sided kernel (n < 8192:
  *     inside one fused launch per nb_step() call).
  *   NB_PATH_ONE_SIDED: every ORDERED pair (i, j) is evaluated; a CTA owns an (i-block, j-split).
  *   NB_PATH_SYMMETRIC: every UNORDERED pair is evaluated once and serves both a_i and a_j

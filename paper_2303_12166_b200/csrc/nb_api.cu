@@ -44,7 +44,7 @@ constexpr int kMaxContactChunks = 32;              // index-order search: the ca
 
 // Force-path selection (nb_set_force_path).
 enum { kPathAuto = 0, kPathOneSided = 1, kPathSymmetric = 2 };
-constexpr int64_t kSymMinN = 10240;               // auto: symmetric kernel from here on.  The kernel alone wins from ~6,000
+constexpr int64_t kSymMinN = 8192;                // auto: symmetric kernel from here on.  The kernel alone wins from ~6,000
                                                   // elements, but its 126 registers leave the contact pass no room to run
                                                   // beside it; measured whole steps (one-sided / symmetric, us): 8,192: 64 / 67,
                                                   // 10,240: 79 / 78, 12,288: 105 / 89, 16,384: 164 / 137, 24,576: 331 / 243
