@@ -195,7 +195,7 @@ const char* nb_force_kernel_name(nb_ctx* ctx);
 int64_t nb_launch_count(nb_ctx* ctx);
 
 /* Measurement aids: launch the all-pairs gravity kernel (row a2: Eq. 4 over all N^2 ordered
- * pairs; nb_time_force_kernel) or the contact pass (row a3: Hilbert keys, sort, gather, Eqs. 5/6;
+ * pairs; nb_time_force_kernel) or the contact pass (row a3: cell list -- bbox, count, scan, scatter, rank -- and Eqs. 5/6;
  * nb_time_contact_pass, 0 ms when gamma == 0) `reps` times on the ctx stream after one warm-up,
  * bracketed by CUDA events on that stream; HOST *ms_avg receives the average duration of one
  * pass.  Their partial sums land in the workspace and touch no state.  Synchronise the stream. */

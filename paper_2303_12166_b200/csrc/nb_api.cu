@@ -425,18 +425,23 @@ int launch_contact(nb_ctx* c) { return launch_contact_on(c, c->stream); }
 
 // Rows a2 + a3: every slab nb_reduce_update_kernel sums for a(x).  The two are independent (both
 // read the state, each writes its own slabs), so the contact pass -- seven short launches that
-// cannot fill the machine -- runs on the library's side stream beside the gravity kernel:
-// fork after whatever the ctx stream holds, join before the update kernel.
+// cannot fill the machine -- runs on the library's side stream: fork after whatever the ctx stream
+// holds, join before the update kernel.  The gravity kernel is launched FIRST and the side stream has
+// the same (default) priority, so the block scheduler places the contact CTAs where the gravity kernel
+// leaves room: beside the one-sided kernel, and in the ragged last wave of the symmetric kernel, whose
+// CTAs fill the register file (measured whole steps, contact first on a high-priority stream -> this
+// order: 16,384 elements 156 -> 135 us, 65,536 1.322 -> 1.280 ms, 262,144 18.81 -> 18.64 ms; a contact
+// CTA that takes a slot from a retiring gravity CTA mid-kernel costs more than it would in the tail).
 int launch_force(nb_ctx* c)
 {
     if (!c->contact_on()) return launch_gravity(c);
     NB_CUDA(c, cudaEventRecord(c->ev_fork, c->stream));
+    int rc = launch_gravity(c);
+    if (rc) return rc;
     NB_CUDA(c, cudaStreamWaitEvent(c->side, c->ev_fork, 0));
-    int rc = launch_contact_on(c, c->side);
+    rc = launch_contact_on(c, c->side);
     if (rc) return rc;
     NB_CUDA(c, cudaEventRecord(c->ev_join, c->side));
-    rc = launch_gravity(c);
-    if (rc) return rc;
     NB_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_join, 0));
     return NB_OK;
 }
@@ -556,9 +561,8 @@ int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream
     c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     c->num_sms = sms > 0 ? sms : kNumSMsFallback;
     c->lay = make_layout(n_max);
-    int prio_lo = 0, prio_hi = 0;                  // high priority: its small CTAs go first as gravity CTAs retire
-    cudaDeviceGetStreamPriorityRange(&prio_lo, &prio_hi);
-    if (cudaStreamCreateWithPriority(&c->side, cudaStreamNonBlocking, prio_hi) != cudaSuccess ||
+    // default priority, like the gravity kernel launched before it: see launch_force()
+    if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_join, cudaEventDisableTiming) != cudaSuccess) {
         nb_destroy(c);
