@@ -133,7 +133,7 @@ Plan make_plan(int64_t n, int num_sms, int path)
     p.njt = (int)((n + p.TJ - 1) / p.TJ);
     const int64_t slots = (int64_t)num_sms * kCtasPerSM;
     int64_t pmax = p.njt >= 2 ? p.njt / 2 : 1;
-    if (n < kCellMinN) pmax = p.njt;                 // small n (one fused launch, see nb_fused.cuh): down to one tile per CTA
+    if (n < kCellMinN) pmax = p.njt;                 // small n (the unfused path: nb_relax, no cooperative launch): down to one tile per CTA
     if (pmax > max_split(n)) pmax = max_split(n);
     double best = 0.0;
     for (int64_t P = 1; P <= pmax; ++P) {
@@ -200,7 +200,8 @@ struct nb_ctx {
     cudaStream_t side = nullptr;          // library-owned: the contact pass runs here, beside the gravity kernel
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int num_sms = kNumSMsFallback;
-    int fused_blocks = 0;                 // co-resident CTAs of nb_fused_step_kernel (cooperative launch); 0: not available
+    bool fused_ok = false;                // cooperative launch + the shared memory of nb_fused_step_kernel are available
+    int fused_blocks = 0, fused_logP = 0; // CTAs of nb_fused_step_kernel for the bound state (0: not available) and its 2^logP pairs per CTA
     float4* posm = nullptr;
     float4* vel = nullptr;
     char* ws = nullptr;
@@ -469,22 +470,38 @@ int launch_fused(nb_ctx* c, int nforce, int open, int close_mode, float4* acc_ou
     FusedArgs f;
     std::memset(&f, 0, sizeof(f));
     const int n = (int)c->n;
-    f.grav.posm = c->posm; f.grav.part = c->part();
-    f.grav.n = n; f.grav.nib = c->plan.nib; f.grav.nsplit = c->plan.nsplit; f.grav.njt = c->plan.njt;
-    f.grav.G = c->prm.G; f.grav.eps = c->prm.eps;
+    f.posm = c->posm; f.vel = c->vel; f.posm2 = c->ps(); f.vel2 = c->vs();      // the contact pass's sorted copies are free here
+    f.acc = c->acc(); f.acc_out = acc_out; f.dev = c->dev();
     f.law.n = n;
     f.law.gamma = c->prm.gamma; f.law.gamma_beta = c->prm.gamma * c->prm.beta;
     f.law.v_dead = c->prm.v_dead; f.law.lens_mode = c->prm.lens_mode;
-    f.posm = c->posm; f.vel = c->vel; f.acc = c->acc(); f.acc_out = acc_out;
-    f.dev = c->dev(); f.n = n; f.n1 = c->n1; f.dt = c->prm.dt;
+    f.n = n; f.n1 = c->n1; f.G = c->prm.G; f.eps = c->prm.eps; f.dt = c->prm.dt;
     f.nforce = nforce; f.open = open; f.close_mode = close_mode;
-    long long blocks = (long long)c->plan.nib * c->plan.nsplit;      // one CTA per work item if they fit
-    if (blocks > c->fused_blocks) blocks = c->fused_blocks;
+    f.logP = c->fused_logP; f.npad = (n + kFusedGroup - 1) & ~(kFusedGroup - 1);
     void* args[] = {&f};
-    NB_CUDA(c, cudaLaunchCooperativeKernel((const void*)nb_fused_step_kernel, dim3((unsigned)blocks), dim3(kThreads), args, 0,
-                                           c->stream));
+    NB_CUDA(c, cudaLaunchCooperativeKernel((const void*)nb_fused_step_kernel, dim3((unsigned)c->fused_blocks), dim3(kFusedThreads),
+                                           args, fused_smem_bytes(n), c->stream));
     c->launches++;
     return NB_OK;
+}
+
+// Shape of the fused kernel for the bound state: the smallest power of two P (packed pairs of elements i per CTA)
+// whose ceil(n / 2P) CTAs are all co-resident (the kernel synchronises grid-wide); fused_blocks = 0 if none is.
+void plan_fused(nb_ctx* c)
+{
+    c->fused_blocks = 0;
+    if (!c->fused_ok || c->n >= kCellMinN) return;
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, nb_fused_step_kernel, kFusedThreads,
+                                                      fused_smem_bytes(c->n)) != cudaSuccess || per_sm < 1) {
+        cudaGetLastError();
+        return;
+    }
+    const int64_t cap = (int64_t)per_sm * c->num_sms;
+    for (int lp = 0; lp <= kFusedMaxLogP; ++lp) {
+        const int64_t blocks = (c->n + (2LL << lp) - 1) / (2LL << lp);
+        if (blocks <= cap) { c->fused_logP = lp; c->fused_blocks = (int)blocks; return; }
+    }
 }
 
 // Chain mode: a turn that never came (it cannot, by the ticket order -- this is the safety net that keeps a bug from
@@ -568,11 +585,12 @@ int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream
         nb_destroy(c);
         return NB_ECUDA;
     }
-    {   // CTAs of the fused small-n kernel that can be resident together (it synchronises grid-wide between its phases)
-        int per_sm = 0, coop = 0;
+    {   // the fused small-n kernel: a cooperative launch with up to ~200 KB of dynamic shared memory
+        int coop = 0;
         cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, dev);
-        if (coop && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, nb_fused_step_kernel, kThreads, 0) == cudaSuccess)
-            c->fused_blocks = per_sm * c->num_sms;
+        c->fused_ok = coop && cudaFuncSetAttribute(nb_fused_step_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                   (int)fused_smem_bytes(kCellMinN - 1)) == cudaSuccess;
+        if (!c->fused_ok) cudaGetLastError();
     }
     *out = c;
     return NB_OK;
@@ -623,6 +641,7 @@ int nb_set_state(nb_ctx* c, int64_t n, float* posm, float* vel, const int32_t* s
     c->vel = reinterpret_cast<float4*>(vel);
     c->plan = make_plan(n, c->num_sms, c->path);
     if ((int64_t)c->nslabs() * n > partial_elems_bound(c->n_max)) return NB_ENOMEM;
+    plan_fused(c);
     c->have_state = true;
     return NB_OK;
 }
@@ -906,6 +925,12 @@ int nb_get_launch_info(nb_ctx* c, int32_t* out4)
 {
     if (!c || !out4) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (fused_path(c)) {                  // one cooperative launch: elements i per CTA, j segments per CTA, CTAs
+        out4[0] = 2 << c->fused_logP;
+        out4[1] = kFusedThreads >> c->fused_logP;
+        out4[2] = out4[3] = c->fused_blocks;
+        return NB_OK;
+    }
     if (c->plan.sym_S) {
         out4[0] = c->plan.sym_S;
         out4[1] = c->plan.T;
@@ -935,6 +960,7 @@ int nb_set_force_path(nb_ctx* c, int path)
 const char* nb_force_kernel_name(nb_ctx* c)
 {
     if (!c || !c->have_state) return "";
+    if (fused_path(c)) return "nb_fused_step_kernel";          // rows a2-a6 in one launch (its loop is the one-sided one)
     if (c->plan.sym_S == 256) return sym_name<256>(c->plan.chain);
     if (c->plan.sym_S == 512) return sym_name<512>(c->plan.chain);
     if (c->plan.sym_S == 1024) return sym_name<1024>(c->plan.chain);
@@ -1003,6 +1029,10 @@ int nb_time_contact_pass(nb_ctx* c, int reps, float* ms_avg)
     if (c && !c->contact_on()) { if (ms_avg) *ms_avg = 0.f; return c->have_state ? NB_OK : NB_ESTATE; }
     return time_launches(c, reps, ms_avg, launch_contact);
 }
+
+#ifdef NB_FUSED_PROF
+int nb_debug_fused_prof(long long* host) { return (int)cudaMemcpyFromSymbol(host, nb::g_fused_prof, sizeof(long long) * 512 * 64); }
+#endif
 
 double nb_roche_lobe_radius(double mass_ratio, double k)
 {

@@ -429,6 +429,38 @@ def test_step_calls_can_be_split(nb):
     _check_traj(nb, w, chunks=[1] * 10)
 
 
+@pytest.mark.parametrize("n1,n2", [(1, 1), (3, 2), (150, 147), (1000, 777), (2600, 2521), (4100, 4091)])
+def test_fused_small_n_kernel_shapes_and_step_counts(nb, n1, n2):
+    """The one-launch kernel of n < 8,192 (nb_fused.cuh) at every CTA shape (1 ... 32 packed pairs per CTA), with
+    odd and even numbers of steps per call: its state ping-pongs between the caller's arrays and a scratch copy,
+    and the last update must land in the caller's arrays whatever the count.  Against the oracle, step by step."""
+    kw = dict(name="fused", seed=11, n1=n1, n2=n2, shape="uniform", radius1=1.0, radius2=0.6,
+              q=0.5, a=1.4, eps=0.01, dt=1e-3, nsteps=0)                       # a = 1.4: the stars overlap
+    w = make_binary(**kw)
+    p = params_f32(w.params)
+    s = _sim(nb, w, p)
+    assert nb.nb_force_kernel_name(s.ctx) == "nb_fused_step_kernel"
+    o = oracle.Sim(w.posm, w.vel, w.star, p)
+    done = 0
+    for k in (1, 2, 3, 4, 1):
+        s.step(k); o.step(k); done += k
+        s.synchronize()
+        x = s.posm.cpu().numpy().astype(np.float64)
+        v = s.vel.cpu().numpy().astype(np.float64)
+        assert nb.nb_get_step(s.ctx)[0] == done
+        assert np.array_equal(x[:, 3], w.posm[:, 3].astype(np.float64))
+        assert np.linalg.norm(x[:, :3] - o.x, axis=1).max() / w.meta["a"] <= POS_TOL
+        assert np.linalg.norm(v[:, :3] - o.v, axis=1).max() / (w.meta["omega"] * w.meta["a"]) <= 5e-2
+    a = s.compute_accel().cpu().numpy().astype(np.float64)[:, :3]              # leaves the state where it is
+    x32, v32 = s.posm.cpu().numpy(), s.vel.cpu().numpy()
+    assert np.array_equal(x32.astype(np.float64), x) and np.array_equal(v32.astype(np.float64), v)
+    ao, _, dl = oracle.accel(x32, v32, x32[:, 3], w.star, p["R_start"], p, want_diag=True)   # the oracle on the GPU's own state
+    an = np.linalg.norm(ao, axis=1)
+    assert np.isfinite(a).all()
+    assert (np.maximum(np.linalg.norm(a - ao, axis=1) - dl, 0.0) <= ACC_TOL * an + 1e-12).all()
+    s.close()
+
+
 def _golden(idx):
     path = os.path.join(GOLDEN, f"config{idx}_step10_sample.txt")
     if not os.path.exists(path):

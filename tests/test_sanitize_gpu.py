@@ -35,7 +35,7 @@ def test_every_force_kernel_small():
     import paper_2303_12166_b200 as nb
     w = _w(1500, 1237, 3)                                   # overlapping stars: cross-star contacts as well
     p = params_f32(w.params)
-    assert "nb_gravity_kernel" in _accel_ok(nb, w, p)                                       # fused small-n kernel
+    assert "nb_fused_step_kernel" in _accel_ok(nb, w, p)                                    # fused small-n kernel
     assert "sym_kernel<256" in _accel_ok(nb, w, p, force_path=nb.NB_PATH_SYMMETRIC)         # + index-order contact pass
     w = _w(5000, 4321, 4)                                   # n >= 8,192: cell list; one-sided and symmetric kernels
     p = params_f32(w.params)
