@@ -199,6 +199,24 @@ def nb_splat(ctx: int, centre: Sequence[float], half_width: float, axis_u: int, 
            "nb_splat", ctx)
 
 
+def write_ppm(path: str, image) -> None:
+    """The headless stand-in for the paper's OpenGL window: the nb_splat() image
+    `[2][H][W]` of element counts as a binary PPM (P6) file -- star 0 in the red channel, star 1 in the blue one,
+    counts clipped at 255, row 0 (smallest v) at the bottom like a plot.  File output only: no arithmetic of the
+    method happens here."""
+    img = image.detach().cpu().numpy() if hasattr(image, "detach") else image
+    if img.ndim != 3 or img.shape[0] != 2:
+        raise ValueError("write_ppm expects the [2][H][W] image of nb_splat")
+    import numpy as np
+    H, W = int(img.shape[1]), int(img.shape[2])
+    rgb = np.zeros((H, W, 3), dtype=np.uint8)
+    rgb[..., 0] = np.minimum(img[0], 255)[::-1]
+    rgb[..., 2] = np.minimum(img[1], 255)[::-1]
+    with open(path, "wb") as f:
+        f.write(b"P6\n%d %d\n255\n" % (W, H))
+        f.write(rgb.tobytes())
+
+
 def nb_get_step(ctx: int):
     step = C.c_int64()
     R = (C.c_float * 2)()

@@ -103,3 +103,21 @@ def test_product_and_oracle_do_not_import_each_other():
             assert '#include "nb' not in text
     wl = open(os.path.join(ROOT, "workloads", "configs.py")).read()
     assert "oracle" not in re.sub(r"#.*|\"\"\".*?\"\"\"", "", wl, flags=re.S) and "paper_2303" not in wl
+
+
+def test_write_ppm_writes_the_splat_image_as_a_p6_file(tmp_path):
+    """the headless image goes to a file (PPM) where the paper opens a window; host-side only."""
+    import numpy as np
+    import paper_2303_12166_b200 as nb
+    img = np.zeros((2, 3, 4), dtype=np.int32)
+    img[0, 0, 1] = 7          # star 0, bottom row
+    img[1, 2, 3] = 300        # star 1, top row, clipped at 255
+    path = tmp_path / "splat.ppm"
+    nb.write_ppm(str(path), img)
+    raw = path.read_bytes()
+    assert raw.startswith(b"P6\n4 3\n255\n")
+    px = np.frombuffer(raw[len(b"P6\n4 3\n255\n"):], dtype=np.uint8).reshape(3, 4, 3)
+    assert px[2, 1].tolist() == [7, 0, 0] and px[0, 3].tolist() == [0, 0, 255] and px.sum() == 7 + 255
+    import pytest
+    with pytest.raises(ValueError):
+        nb.write_ppm(str(path), np.zeros((3, 4), dtype=np.int32))
