@@ -465,7 +465,7 @@ int launch_update(nb_ctx* c, const float4* src, int nsrc, float4* acc_out, float
 // n < kCellMinN: rows a2-a6 for `nforce` force evaluations in ONE cooperative launch (nb_fused.cuh).
 bool fused_path(const nb_ctx* c) { return c->n < kCellMinN && !c->plan.sym_S && c->fused_blocks > 0; }
 
-int launch_fused(nb_ctx* c, int nforce, int open, int close_mode, float4* acc_out)
+int launch_fused(nb_ctx* c, int nforce, int open, int close_mode, float4* acc_out, bool relax = false, float vscale = 1.f)
 {
     FusedArgs f;
     std::memset(&f, 0, sizeof(f));
@@ -476,7 +476,7 @@ int launch_fused(nb_ctx* c, int nforce, int open, int close_mode, float4* acc_ou
     f.law.gamma = c->prm.gamma; f.law.gamma_beta = c->prm.gamma * c->prm.beta;
     f.law.v_dead = c->prm.v_dead; f.law.lens_mode = c->prm.lens_mode;
     f.n = n; f.n1 = c->n1; f.G = c->prm.G; f.eps = c->prm.eps; f.dt = c->prm.dt;
-    f.nforce = nforce; f.open = open; f.close_mode = close_mode;
+    f.nforce = nforce; f.open = open; f.close_mode = close_mode; f.relax = relax ? 1 : 0; f.vscale = vscale;
     f.logP = c->fused_logP; f.npad = (n + kFusedGroup - 1) & ~(kFusedGroup - 1);
     void* args[] = {&f};
     NB_CUDA(c, cudaLaunchCooperativeKernel((const void*)nb_fused_step_kernel, dim3((unsigned)c->fused_blocks), dim3(kFusedThreads),
@@ -703,6 +703,7 @@ int nb_relax(nb_ctx* c, int nsteps, float kappa)
     if (!(f > 0.f)) f = 0.f;
     int rc = ensure_acc(c);
     if (rc) return rc;
+    if (fused_path(c)) return launch_fused(c, nsteps, 1, 0, nullptr, true, f);   // all nsteps in one launch
     for (int s = 0; s < nsteps; ++s) {
         rc = launch_update(c, c->acc(), 1, nullptr, 0.5f * dt, dt, 1);          // half kick, drift, n += 1
         if (rc) return rc;

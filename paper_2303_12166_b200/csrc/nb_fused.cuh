@@ -71,6 +71,8 @@ struct FusedArgs {
     int nforce;                // force evaluations (>= 1)
     int open;                  // 1: start with the opening half kick + drift from the cached acceleration
     int close_mode;            // 0: the last update is the closing half kick; 1: it stores a(x) and moves nothing
+    int relax;                 // 1: nb_relax (row f2, reading A17): the two half kicks of consecutive steps are NOT merged,
+    float vscale;              //    the velocity is multiplied by vscale between them: v <- vscale (v + dt/2 a)
     int logP;                  // 2^logP packed pairs of elements i per CTA
     int npad;                  // n rounded up to a multiple of 8 (whole groups of elements j)
 };
@@ -157,10 +159,16 @@ nb_fused_step_kernel(const __grid_constant__ FusedArgs f)
     float4 *xs = f.posm, *vs = f.vel, *xd = f.posm2, *vd = f.vel2;
     auto swap_buffers = [&]() { float4* t = xs; xs = xd; xd = t; t = vs; vs = vd; vd = t; };
 
-    // element eu, given a: v += kick_h a ; x += drift_dt v, read from (xs, vs), written to (xo, vo)
-    auto move = [&](float ax, float ay, float az, float kick_h, float drift_dt, float4* xo, float4* vo) {
+    // element eu, given a: v += kick_h a ; [v *= scale ; v += kick2_h a] ; x += drift_dt v, read from (xs, vs),
+    // written to (xo, vo)
+    auto move = [&](float ax, float ay, float az, float kick_h, float drift_dt, float4* xo, float4* vo,
+                    bool damp = false, float kick2_h = 0.f) {
         float4 v = __ldcg(vs + eu), p = __ldcg(xs + eu);
         v.x = fmaf(kick_h, ax, v.x); v.y = fmaf(kick_h, ay, v.y); v.z = fmaf(kick_h, az, v.z);
+        if (damp) {
+            if (f.vscale != 1.f) { v.x *= f.vscale; v.y *= f.vscale; v.z *= f.vscale; }
+            if (kick2_h != 0.f) { v.x = fmaf(kick2_h, ax, v.x); v.y = fmaf(kick2_h, ay, v.y); v.z = fmaf(kick2_h, az, v.z); }
+        }
         if (drift_dt != 0.f) {
             p.x = fmaf(drift_dt, v.x, p.x); p.y = fmaf(drift_dt, v.y, p.y); p.z = fmaf(drift_dt, v.z, p.z);
         }
@@ -339,10 +347,11 @@ nb_fused_step_kernel(const __grid_constant__ FusedArgs f)
             }
             const float fax = (float)sxx, fay = (float)syy, faz = (float)szz;
             // U
-            if (!last) {                             // two half kicks merged: v += dt a ; x += dt v
-                move(fax, fay, faz, f.dt, f.dt, xd, vd);
-            } else if (f.close_mode == 0) {          // closing half kick; cache a(x_n)
-                move(fax, fay, faz, 0.5f * f.dt, 0.f, xd, vd);
+            if (!last) {
+                if (f.relax) move(fax, fay, faz, 0.5f * f.dt, f.dt, xd, vd, true, 0.5f * f.dt);   // half kick, damp, half kick, drift
+                else         move(fax, fay, faz, f.dt, f.dt, xd, vd);   // two half kicks merged: v += dt a ; x += dt v
+            } else if (f.close_mode == 0) {          // closing half kick (nb_relax: then v <- vscale v); cache a(x_n)
+                move(fax, fay, faz, 0.5f * f.dt, 0.f, xd, vd, f.relax != 0);
                 f.acc[eu] = make_float4(fax, fay, faz, 0.f);
             } else {                                 // a(x) only
                 f.acc[eu] = make_float4(fax, fay, faz, 0.f);

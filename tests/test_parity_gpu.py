@@ -459,6 +459,18 @@ def test_fused_small_n_kernel_shapes_and_step_counts(nb, n1, n2):
     assert np.isfinite(a).all()
     assert (np.maximum(np.linalg.norm(a - ao, axis=1) - dl, 0.0) <= ACC_TOL * an + 1e-12).all()
     s.close()
+    s = _sim(nb, w, p)                                                          # nb_relax takes the same kernel (row f2);
+    o = oracle.Sim(w.posm, w.vel, w.star, p)                                    # fresh pair: the parity horizon is 10 steps (A16)
+    done = 0
+    for k, kappa in ((3, 30.0), (2, 0.0), (1, 400.0)):
+        s.relax(k, kappa); o.relax(k, kappa); done += k
+        s.synchronize()
+        x = s.posm.cpu().numpy().astype(np.float64)
+        v = s.vel.cpu().numpy().astype(np.float64)
+        assert nb.nb_get_step(s.ctx)[0] == done
+        assert np.linalg.norm(x[:, :3] - o.x, axis=1).max() / w.meta["a"] <= POS_TOL
+        assert np.linalg.norm(v[:, :3] - o.v, axis=1).max() / (w.meta["omega"] * w.meta["a"]) <= 5e-2
+    s.close()
 
 
 def _golden(idx):
