@@ -113,7 +113,8 @@ int nb_energy(nb_ctx* ctx, double* out);
  * f2, star construction (elements are put together and "this technique was used to
  * create a binary system"; no procedure is printed -- reading A17): nsteps leapfrog steps as in
  * nb_step(), each followed by v <- max(0, 1 - kappa*dt) v, so a star (or the binary) settles
- * into equilibrium.  kappa >= 0 [1/time]; kappa = 0 is nb_step() exactly.  The step count and the
+ * into equilibrium.  kappa >= 0 [1/time]; kappa = 0 is nb_step() up to fp32 rounding (nb_step merges the two
+ * half kicks of consecutive steps into one multiply-add, nb_relax cannot).  The step count and the
  * radius ramp advance as usual.  Asynchronous on the stream. */
 int nb_relax(nb_ctx* ctx, int nsteps, float kappa);
 
@@ -165,12 +166,16 @@ int nb_download_state(nb_ctx* ctx, float* host_posm, float* host_vel, float* hos
 /* Launch configuration chosen for the bound state (for reports): i-elements per
  * CTA, j-splits P, CTAs of the force kernel, CTAs of the update kernel (one-sided kernel);
  * super-tile size S, super-tiles T (= partial-sum slabs), CTAs = T(T+1)/2, CTAs of the update
- * kernel (symmetric kernel). */
+ * kernel (symmetric kernel); elements i per CTA, j segments per CTA, CTAs, CTAs (n < 8192: the
+ * one cooperative launch that runs whole steps). */
 int nb_get_launch_info(nb_ctx* ctx, int32_t* out4);
 
 /* Which kernel evaluates row a2 (Eq. 4, summed over all pairs).
- *   NB_PATH_AUTO (default): the symmetric kernel for n >= 8192, else the one-sided kernel (n < 8192:
- *     inside one fused launch per nb_step() call).
+ *   NB_PATH_AUTO (default): the symmetric kernel for n >= 8192; for n < 8192 the one-sided loop inside
+ *     nb_fused_step_kernel: ONE cooperative launch per nb_step() / nb_relax() / nb_compute_accel() call runs
+ *     rows a2-a6 for all its steps (every CTA owns a slice of elements i; the state ping-pongs between the
+ *     caller's arrays and workspace scratch inside the launch and is back in the caller's arrays at its end).
+ *     NB_PATH_ONE_SIDED takes the same launch for n < 8192.
  *   NB_PATH_ONE_SIDED: every ORDERED pair (i, j) is evaluated; a CTA owns an (i-block, j-split).
  *   NB_PATH_SYMMETRIC: every UNORDERED pair is evaluated once and serves both a_i and a_j
  *     (the force of Eq. 4 is "between elements i and j": F_ij = -F_ji); a CTA owns a pair of
