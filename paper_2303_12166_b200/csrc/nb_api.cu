@@ -147,7 +147,7 @@ Plan make_plan(int64_t n, int num_sms, int path)
 
 struct Layout {
     size_t off_dev, off_acc, off_part, off_red, off_ps, off_vs, off_gbox, off_sbox, off_cpart, off_cstate,
-        off_counters, off_bsum, off_bucket, off_slot, off_tmp, off_perm, off_acc64, off_turn, off_epot, off_erep, total;
+        off_counters, off_bsum, off_bucket, off_slot, off_tmp, off_perm, off_acc64, off_turn, off_epot, off_erep, off_tbox, total;
 };
 
 // Super-tile of nb_pot_pair_kernel for n elements (T <= 512 up to 2M elements), and its CTAs = fp64 partials.
@@ -186,6 +186,7 @@ Layout make_layout(int64_t n_max)
     L.off_turn = o;     o += align_up(n_max >= kChainMinN ? ((size_t)(n_max / 1024 + 1) * 5 + 2) * sizeof(int) : 0);   // <= 4 rounds + 1 per tile
     L.off_epot = o;     o += align_up((size_t)pot_pairs(n_max) * sizeof(double));
     L.off_erep = o;     o += align_up(((size_t)n_max * 4 / kCcThreads + 1) * sizeof(double));
+    L.off_tbox = o;     o += align_up(((size_t)n_max / 1024 + 1) * 2 * sizeof(float4));   // nb_energy: boxes of its super-tiles (S >= 1,024)
     L.total = o;
     return L;
 }
@@ -827,12 +828,26 @@ int nb_energy(nb_ctx* c, double* out)
     double *dpot = nullptr, *drep = nullptr;
     const bool big = c->n >= kCellMinN;
     if (big) {                                       // packed pair-of-super-tiles kernel + the cell list in energy mode
+        // U_rep first: the cell list in energy mode, which also leaves the elements in cell order (ps, vs) -- the
+        // order in which most pairs of super-tiles are far apart (nb_pot_pair_kernel)
+        if (c->contact_on()) {
+            drep = c->at<double>(c->lay.off_erep);
+            nrep = (size_t)((((long long)n << (c->n < kContactWideN ? 2 : 0)) + kCcThreads - 1) / kCcThreads);
+            rc = launch_contact_on(c, c->stream, drep);
+            if (rc) return rc;
+        }
         PotPairArgs pa;
-        pa.posm = c->posm; pa.out = dpot = c->at<double>(c->lay.off_epot);
+        pa.px = c->contact_on() ? c->ps() : c->posm;
+        pa.pm = c->contact_on() ? c->vs() : c->posm;
+        pa.out = dpot = c->at<double>(c->lay.off_epot);
         pa.n = n; pa.G = c->prm.G; pa.eps = c->prm.eps;
         const int S = pot_tile(c->n);
         pa.T = (int)((c->n + S - 1) / S);
         npot = (size_t)pot_pairs(c->n);
+        float4* tbox = c->at<float4>(c->lay.off_tbox);
+        pa.box = tbox;
+        nb_tile_bbox_kernel<<<pa.T, 256, 0, c->stream>>>(pa.px, n, S, tbox);
+        c->launches++;
         if (S == 1024)      nb_pot_pair_kernel<1024, 8, 128><<<(unsigned)npot, 128, 16 * 1024, c->stream>>>(pa);
         else if (S == 4096) {
             static bool cfg = false;
@@ -845,12 +860,6 @@ int nb_energy(nb_ctx* c, double* out)
         }
         c->launches++;
         NB_CUDA(c, cudaGetLastError());
-        if (c->contact_on()) {
-            drep = c->at<double>(c->lay.off_erep);
-            nrep = (size_t)((((long long)n << (c->n < kContactWideN ? 2 : 0)) + kCcThreads - 1) / kCcThreads);
-            rc = launch_contact_on(c, c->stream, drep);
-            if (rc) return rc;
-        }
     } else {
         const int pot_blocks = (n + kThreads - 1) / kThreads;
         PotArgs pa;

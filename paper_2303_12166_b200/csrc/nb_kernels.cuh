@@ -1261,24 +1261,66 @@ nb_potential_kernel(const __grid_constant__ PotArgs a)
 
 // Row a7 for n >= 8,192: U_grav = -sum_{i<j} G m_i m_j / (r + eps) over pairs of super-tiles (A <= B), one CTA each,
 // in the packed form of the symmetric gravity kernel: B staged in shared memory as packed pairs (broadcast LDS.64),
-// NI elements i of A per lane, per pair one MUFU.RSQ (r = r^2 y) and one MUFU.RCP (1/(r + eps)) -- the XU pipe bounds
-// it at the same N^2 MUFU as a force evaluation.  fp32 terms in chains of <= 128, flushed into fp64; one fp64
-// partial per CTA, summed on the host in CTA order.  A diagonal CTA (A == B) counts every ordered pair but the
-// self pair (masked by index) and halves the sum.  U_rep comes from the cell list (nb_cells.cuh, energy mode).
+// NI elements i of A per lane, per pair one MUFU.RSQ (y = 1/r, r = r^2 y) and
+//   near pairs of super-tiles: one MUFU.RCP, 1/(r + eps) -- the XU pipe bounds them at the N^2 MUFU of a force evaluation;
+//   FAR pairs (bounding boxes at least 100 eps apart, so u = eps/r <= 0.01): no second MUFU, the factor 1/(1 + u) as
+//   1 - u + u^2 - u^3 (truncation error u^4 <= 1e-8 relative), i.e. y (1 + y (-eps + y (eps^2 - eps^3 y))): three FFMA2 and
+//   one FMUL2 instead -- the FMA pipe bounds them, at 22 instead of 32 cycles per packed evaluation.
+// The elements are taken in the cell-list order of the contact pass when there is one (nb_energy runs it first, in
+// energy mode): super-tiles are then thin pencils of cells and ~90 % of the same-star pairs are far as well; in the
+// caller's order only the pairs of super-tiles from different stars are.  Either way the sum is over the same pairs.
+// fp32 terms in chains of <= 128, flushed into fp64; one fp64 partial per CTA, summed on the host in CTA order.  A
+// diagonal CTA (A == B) counts every ordered pair but the self pair (masked by index) and halves the sum.
+// U_rep comes from the cell list (nb_cells.cuh, energy mode).
 struct PotPairArgs {
-    const float4* __restrict__ posm;   // [n] x,y,z,m
+    const float4* __restrict__ px;     // [n] x,y,z,.   (posm, or the sorted copy ps)
+    const float4* __restrict__ pm;     // [n] .,.,.,m   (posm, or the sorted copy vs)
+    const float4* __restrict__ box;    // [T][2] bounding box of every super-tile (lo, hi)
     double* __restrict__ out;          // [T (T + 1) / 2]
     int n, T;
     float G, eps;
 };
 
-template <int NI, bool DIAG>
+// Bounding boxes of the super-tiles of S elements: one block per super-tile.
+__global__ void __launch_bounds__(256)
+nb_tile_bbox_kernel(const float4* __restrict__ px, int n, int S, float4* __restrict__ box)
+{
+    __shared__ float sh[6][8];
+    const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+    float lo[3] = {3.0e38f, 3.0e38f, 3.0e38f}, hi[3] = {-3.0e38f, -3.0e38f, -3.0e38f};
+    const long long e0 = (long long)blockIdx.x * S;
+    for (int k = threadIdx.x; k < S && e0 + k < n; k += 256) {
+        const float4 q = px[e0 + k];
+        lo[0] = fminf(lo[0], q.x); lo[1] = fminf(lo[1], q.y); lo[2] = fminf(lo[2], q.z);
+        hi[0] = fmaxf(hi[0], q.x); hi[1] = fmaxf(hi[1], q.y); hi[2] = fmaxf(hi[2], q.z);
+    }
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+        const float a = warp_min(lo[c]), b = warp_max(hi[c]);
+        if (l == 0) { sh[c][w] = a; sh[3 + c][w] = b; }
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        float q[6];
+        for (int c = 0; c < 3; ++c) {
+            q[c] = sh[c][0]; q[3 + c] = sh[3 + c][0];
+            for (int k = 1; k < 8; ++k) { q[c] = fminf(q[c], sh[c][k]); q[3 + c] = fmaxf(q[3 + c], sh[3 + c][k]); }
+        }
+        box[2 * blockIdx.x] = make_float4(q[0], q[1], q[2], 0.f);
+        box[2 * blockIdx.x + 1] = make_float4(q[3], q[4], q[5], 0.f);
+    }
+}
+
+constexpr float kPotFarGap = 100.f;    // a pair of super-tiles is FAR if its boxes are at least this many eps apart
+
+template <int NI, bool DIAG, bool FAR>
 __device__ __forceinline__ void pot_step(const f32x2 X, const f32x2 Y, const f32x2 Z, const f32x2 M, const int j0,
                                          const float (&nxi)[NI], const float (&nyi)[NI], const float (&nzi)[NI],
-                                         const int (&ei)[NI], const f32x2 eps2, f32x2 (&acc)[NI])
+                                         const int (&ei)[NI], const f32x2 eps2, const f32x2 neps, const f32x2 e2,
+                                         const f32x2 ne3, f32x2 (&acc)[NI])
 {
     const f32x2 tiny2 = pk2(kTinyR2, kTinyR2);
-    f32x2 r2[NI], y[NI], sm[NI];
+    f32x2 r2[NI], y[NI];
 #pragma unroll
     for (int i = 0; i < NI; ++i) {
         const f32x2 dx = add2(X, pk2(nxi[i], nxi[i])), dy = add2(Y, pk2(nyi[i], nyi[i])), dz = add2(Z, pk2(nzi[i], nzi[i]));
@@ -1290,20 +1332,80 @@ __device__ __forceinline__ void pot_step(const f32x2 X, const f32x2 Y, const f32
         unpk2(r2[i], a0, b0);
         y[i] = pk2(rsqrt_approx(a0), rsqrt_approx(b0));
     }
+    if constexpr (FAR) {                             // 1/(r + eps) = y / (1 + eps y) = y (1 + y (-eps + y (eps^2 - eps^3 y)))
+        const f32x2 one = pk2(1.f, 1.f);
 #pragma unroll
-    for (int i = 0; i < NI; ++i) sm[i] = fma2(r2[i], y[i], eps2);                 // r + eps
-#pragma unroll
-    for (int i = 0; i < NI; ++i) {
-        float a0, b0;
-        unpk2(sm[i], a0, b0);
-        f32x2 w = M;
-        if (DIAG) {                                  // the self pair does not count
-            float m0, m1;
-            unpk2(M, m0, m1);
-            w = pk2(j0 == ei[i] ? 0.f : m0, j0 + 1 == ei[i] ? 0.f : m1);
+        for (int i = 0; i < NI; ++i) {
+            f32x2 q = fma2(y[i], ne3, e2);
+            q = fma2(y[i], q, neps);
+            q = fma2(y[i], q, one);
+            acc[i] = fma2(M, mul2(y[i], q), acc[i]);                                  // m_j / (r + eps)
         }
-        acc[i] = fma2(w, pk2(rcp_approx(a0), rcp_approx(b0)), acc[i]);            // m_j / (r + eps)
+    } else {
+        f32x2 sm[NI];
+#pragma unroll
+        for (int i = 0; i < NI; ++i) sm[i] = fma2(r2[i], y[i], eps2);             // r + eps
+#pragma unroll
+        for (int i = 0; i < NI; ++i) {
+            float a0, b0;
+            unpk2(sm[i], a0, b0);
+            f32x2 w = M;
+            if (DIAG) {                              // the self pair does not count
+                float m0, m1;
+                unpk2(M, m0, m1);
+                w = pk2(j0 == ei[i] ? 0.f : m0, j0 + 1 == ei[i] ? 0.f : m1);
+            }
+            acc[i] = fma2(w, pk2(rcp_approx(a0), rcp_approx(b0)), acc[i]);        // m_j / (r + eps)
+        }
     }
+}
+
+// MODE 0: off-diagonal pair of super-tiles, near; 1: diagonal; 2: off-diagonal, far.
+template <int S, int NI, int NT, int MODE>
+__device__ __forceinline__ double pot_sweep(const PotPairArgs& a, const int A, const int B,
+                                            const float2* __restrict__ X2, const float2* __restrict__ Y2,
+                                            const float2* __restrict__ Z2, const float2* __restrict__ M2)
+{
+    constexpr int IPR = NT * NI;                     // elements i per round
+    const int tid = threadIdx.x;
+    const f32x2 eps2 = pk2(a.eps, a.eps), neps = pk2(-a.eps, -a.eps), e2 = pk2(a.eps * a.eps, a.eps * a.eps),
+                ne3 = pk2(-a.eps * a.eps * a.eps, -a.eps * a.eps * a.eps);
+    double total = 0.0;
+#pragma unroll 1
+    for (int r = 0; r < S / IPR; ++r) {
+        float nxi[NI], nyi[NI], nzi[NI], mi[NI];
+        int ei[NI];
+        double phi[NI];
+#pragma unroll
+        for (int i = 0; i < NI; ++i) {
+            ei[i] = A * S + r * IPR + i * NT + tid;
+            float4 q = make_float4(-kFarAway, -kFarAway, -kFarAway, 0.f);
+            if (ei[i] < a.n) { q = a.px[ei[i]]; q.w = a.pm[ei[i]].w; }
+            nxi[i] = -q.x; nyi[i] = -q.y; nzi[i] = -q.z; mi[i] = q.w;
+            phi[i] = 0.0;
+        }
+#pragma unroll 1
+        for (int p0 = 0; p0 < S / 2; p0 += 64) {
+            f32x2 acc[NI];
+#pragma unroll
+            for (int i = 0; i < NI; ++i) acc[i] = pk2(0.f, 0.f);
+#pragma unroll 4
+            for (int p = p0; p < p0 + 64; ++p) {
+                const f32x2 X = *reinterpret_cast<const f32x2*>(X2 + p), Y = *reinterpret_cast<const f32x2*>(Y2 + p),
+                            Z = *reinterpret_cast<const f32x2*>(Z2 + p), M = *reinterpret_cast<const f32x2*>(M2 + p);
+                pot_step<NI, MODE == 1, MODE == 2>(X, Y, Z, M, B * S + 2 * p, nxi, nyi, nzi, ei, eps2, neps, e2, ne3, acc);
+            }
+#pragma unroll
+            for (int i = 0; i < NI; ++i) {
+                float l, h;
+                unpk2(acc[i], l, h);
+                phi[i] += (double)l + (double)h;
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < NI; ++i) total += (double)mi[i] * phi[i];
+    }
+    return total;
 }
 
 template <int S, int NI, int NT>
@@ -1316,8 +1418,7 @@ nb_pot_pair_kernel(const __grid_constant__ PotPairArgs a)
     float2* __restrict__ Y2 = X2 + S / 2;
     float2* __restrict__ Z2 = Y2 + S / 2;
     float2* __restrict__ M2 = Z2 + S / 2;
-    constexpr int IPR = NT * NI;                     // elements i per round
-    static_assert(S % IPR == 0 && (S / 2) % 64 == 0, "whole rounds; whole flush intervals");
+    static_assert(S % (NT * NI) == 0 && (S / 2) % 64 == 0, "whole rounds; whole flush intervals");
     const int tid = threadIdx.x;
     int A, B;
     {
@@ -1336,50 +1437,21 @@ nb_pot_pair_kernel(const __grid_constant__ PotPairArgs a)
     for (int p = tid; p < S / 2; p += NT) {          // pair p holds elements 2 p and 2 p + 1 of B
         const int e0 = B * S + 2 * p, e1 = e0 + 1;
         float4 q0 = make_float4(kFarAway, kFarAway, kFarAway, 0.f), q1 = q0;
-        if (e0 < a.n) q0 = a.posm[e0];
-        if (e1 < a.n) q1 = a.posm[e1];
+        if (e0 < a.n) { q0 = a.px[e0]; q0.w = a.pm[e0].w; }
+        if (e1 < a.n) { q1 = a.px[e1]; q1.w = a.pm[e1].w; }
         X2[p] = make_float2(q0.x, q1.x); Y2[p] = make_float2(q0.y, q1.y); Z2[p] = make_float2(q0.z, q1.z);
         M2[p] = make_float2(q0.w, q1.w);
     }
     __syncthreads();
-    const f32x2 eps2 = pk2(a.eps, a.eps);
-    double total = 0.0;
-#pragma unroll 1
-    for (int r = 0; r < S / IPR; ++r) {
-        float nxi[NI], nyi[NI], nzi[NI], mi[NI];
-        int ei[NI];
-        double phi[NI];
-#pragma unroll
-        for (int i = 0; i < NI; ++i) {
-            ei[i] = A * S + r * IPR + i * NT + tid;
-            float4 q = make_float4(-kFarAway, -kFarAway, -kFarAway, 0.f);
-            if (ei[i] < a.n) q = a.posm[ei[i]];
-            nxi[i] = -q.x; nyi[i] = -q.y; nzi[i] = -q.z; mi[i] = q.w;
-            phi[i] = 0.0;
-        }
-#pragma unroll 1
-        for (int p0 = 0; p0 < S / 2; p0 += 64) {
-            f32x2 acc[NI];
-#pragma unroll
-            for (int i = 0; i < NI; ++i) acc[i] = pk2(0.f, 0.f);
-#pragma unroll 4
-            for (int p = p0; p < p0 + 64; ++p) {
-                const f32x2 X = *reinterpret_cast<const f32x2*>(X2 + p), Y = *reinterpret_cast<const f32x2*>(Y2 + p),
-                            Z = *reinterpret_cast<const f32x2*>(Z2 + p), M = *reinterpret_cast<const f32x2*>(M2 + p);
-                if (A == B) pot_step<NI, true>(X, Y, Z, M, B * S + 2 * p, nxi, nyi, nzi, ei, eps2, acc);
-                else        pot_step<NI, false>(X, Y, Z, M, 0, nxi, nyi, nzi, ei, eps2, acc);
-            }
-#pragma unroll
-            for (int i = 0; i < NI; ++i) {
-                float l, h;
-                unpk2(acc[i], l, h);
-                phi[i] += (double)l + (double)h;
-            }
-        }
-#pragma unroll
-        for (int i = 0; i < NI; ++i) total += (double)mi[i] * phi[i];
-    }
-    total *= (A == B ? 0.5 : 1.0) * (double)a.G;
+    // far: every r of the pair of super-tiles is at least kPotFarGap eps (and more than nothing)
+    const float gap2 = box_gap2(a.box[2 * A], a.box[2 * A + 1], a.box[2 * B], a.box[2 * B + 1]);
+    const float need = kPotFarGap * a.eps;
+    const bool far = A != B && gap2 > 0.f && gap2 >= need * need;
+    double total;
+    if (A == B)   total = 0.5 * pot_sweep<S, NI, NT, 1>(a, A, B, X2, Y2, Z2, M2);
+    else if (far) total = pot_sweep<S, NI, NT, 2>(a, A, B, X2, Y2, Z2, M2);
+    else          total = pot_sweep<S, NI, NT, 0>(a, A, B, X2, Y2, Z2, M2);
+    total *= (double)a.G;
     const double rsum = block_sum(total, sh);
     if (tid == 0) a.out[blockIdx.x] = rsum;
 }
