@@ -549,11 +549,19 @@ def _energy_case(kind):
         return w, 0
     if kind == "config3_after_ramp_steps":    # N = 65,536, cross-star radii differ after 10 ramp steps
         return make_config(3), 10
+    if kind == "gamma0_callers_order":        # no contact terms -> no cell list: U_grav in the caller's order, where only the
+        w = _ragged(12000, 9001, seed=46)     # pairs of super-tiles from different stars are far (series in eps/r)
+        w.params["gamma"] = 0.0
+        return w, 0
+    if kind == "eps0_far_pairs":              # eps = 0: the series is exact, every separated pair of super-tiles is far
+        w = _ragged(9000, 7000, seed=47)
+        w.params["eps"] = 0.0
+        return w, 0
     raise KeyError(kind)
 
 
 @pytest.mark.parametrize("kind", ["config1", "n2049", "ragged_9321", "tiny_129_1", "n512_255_257", "config2_lognormal",
-                                  "sym_24576_mixed", "config3_after_ramp_steps"])
+                                  "sym_24576_mixed", "config3_after_ramp_steps", "gamma0_callers_order", "eps0_far_pairs"])
 def test_energy_and_momenta_match_oracle(nb, kind):
     """nb_energy against orc_energy on the GPU's own state (so that only the diagnostic is compared, not the
     trajectory): ragged sizes, lognormal masses, the star boundary inside a tile, both gravity paths' sizes, and
