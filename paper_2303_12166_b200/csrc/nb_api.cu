@@ -223,7 +223,12 @@ struct nb_ctx {
     float4* gbox() const { return reinterpret_cast<float4*>(ws + lay.off_gbox); }
     float4* sbox() const { return reinterpret_cast<float4*>(ws + lay.off_sbox); }
     template <class T> T* at(size_t off) const { return reinterpret_cast<T*>(ws + off); }
-    bool contact_on() const { return prm.gamma > 0.f; }
+    // contact terms exist: gamma > 0 and some element has a radius at some step (with every radius 0 for good no pair can
+    // touch, and the cell list would put a whole star into one cell)
+    bool contact_on() const {
+        return prm.gamma > 0.f && (prm.R_start[0] > 0.f || prm.R_start[1] > 0.f ||
+                                   (prm.n_ramp > 0 && (prm.R_end[0] > 0.f || prm.R_end[1] > 0.f)));
+    }
     int ngrav() const { return plan.sym_S ? (plan.chain ? 0 : plan.T) : plan.nsplit; }   // gravity slabs
     int ncontact() const {                                                // contact slabs
         if (!contact_on()) return 0;

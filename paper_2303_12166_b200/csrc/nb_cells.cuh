@@ -206,6 +206,10 @@ __device__ __forceinline__ CellGrid cell_make_grid(const CellPartial* __restrict
         if (m[2] > m[c]) c = 2;
         m[c] >>= 1;
     }
+    if (!(g.inv_h > 0.f)) {                                      // no reach (every radius 0 at this step): nobody will query
+        m[1] = m[2] = kCellMinDim;                               // this grid; the elements are dealt over all its buckets
+        m[0] = (cap > 64 ? cap : 64) / (kCellMinDim * kCellMinDim);   // by index (cell_phase_count), not piled into one
+    }
     g.mx = m[0] - 1; g.my = m[1] - 1; g.mz = m[2] - 1;
     g.sy = 31 - __clz(m[0]); g.sz = g.sy + 31 - __clz(m[1]);
     g.base = base; g.count = cnt;
@@ -228,8 +232,12 @@ __device__ __forceinline__ void cell_phase_count(const CellPassArgs& a, CellGrid
     for (int i = blockIdx.x * kPassThreads + threadIdx.x; i < a.n; i += gridDim.x * kPassThreads) {
         const float4 p = a.posm[i];
         const CellGrid& g = sg[i < a.n1 ? 0 : 1];
-        const int b = cell_bucket(g, cell_coord(p.x, g.org[0], g.inv_h), cell_coord(p.y, g.org[1], g.inv_h),
-                                  cell_coord(p.z, g.org[2], g.inv_h));
+        int b;
+        if (g.inv_h > 0.f)
+            b = cell_bucket(g, cell_coord(p.x, g.org[0], g.inv_h), cell_coord(p.y, g.org[1], g.inv_h),
+                            cell_coord(p.z, g.org[2], g.inv_h));
+        else                                                     // a grid without reach: one element per bucket, by index
+            b = g.base + ((i < a.n1 ? i : i - a.n1) & ((g.mx + 1) * (g.my + 1) * (g.mz + 1) - 1));   // (a power of two >= 2 n_s)
         a.bucket[i] = b;
         a.slot[i] = atomicAdd(&a.counters[b], 1);
     }

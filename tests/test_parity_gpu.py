@@ -335,6 +335,27 @@ def test_cell_list_tests_few_candidates_per_element(nb, idx):
     assert abs(st["queued"] / w.n - cnt.mean()) <= 4.0 * cnt.std() / np.sqrt(len(rows)) + 0.01
 
 
+def test_zero_radii_with_contact_strength_set(nb):
+    """gamma > 0 but every element radius 0 (for good, or at the start of a ramp from 0): no pair can touch, the
+    result is gravity alone, and the cell list must not pile a whole star into one cell (its re-ranking would be
+    quadratic): the evaluation has to come back promptly at 60,000 elements."""
+    import time
+    w = _ragged(40000, 20000, seed=21)
+    for over in (dict(R_start=(0.0, 0.0), R_end=(0.0, 0.0), n_ramp=0),
+                 dict(R_start=(0.0, 0.0), R_end=(0.02, 0.015), n_ramp=100)):
+        p = params_f32(dict(w.params, **over))
+        p0 = dict(p); p0["gamma"] = 0.0
+        t0 = time.perf_counter()
+        a, _ = _gpu_accel(nb, w, p)
+        dt = time.perf_counter() - t0
+        a0, _ = _gpu_accel(nb, w, p0)
+        assert np.array_equal(a, a0)
+        assert dt < 5.0, dt
+        rows = _sample(w.n, 256, 3)
+        ao = oracle.accel(w.posm, w.vel, w.posm[:, 3], w.star, p["R_start"], p, rows=rows)
+        assert (np.linalg.norm(a[rows] - ao, axis=1) <= ACC_TOL * np.linalg.norm(ao, axis=1)).all()
+
+
 def test_contact_pass_timing_entry_point(nb):
     w = make_config(2)
     p = params_f32(w.params)
