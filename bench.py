@@ -389,6 +389,9 @@ def run_own(args):
                 "traffic_model": {"slab_bytes_written": float(nslab) * n * 16, "slabs": nslab,
                                   "note": "partial sums the kernel writes once per launch (ALU-bound: HBM is not the limit)"},
                 "kernel": kernel, "kernel_ms": k_ms,
+                **({"kernel_ms_note": "n < 8192: the step runs in ONE cooperative launch (nb_fused_step_kernel); kernel_ms and "
+                                      "contact_pass_ms time the stand-alone one-sided gravity kernel and index-order contact "
+                                      "pass of the unfused path, for orientation only"} if "fused" in kernel else {}),
                 "executed_flop_per_interaction": executed, "flop_per_interaction": FLOP_PER_INTERACTION,
                 "pair_evaluations": "each unordered pair once (Newton's third law)" if symmetric
                                     else "every ordered pair",
