@@ -44,10 +44,10 @@ constexpr int kMaxContactChunks = 32;              // index-order search: the ca
 
 // Force-path selection (nb_set_force_path).
 enum { kPathAuto = 0, kPathOneSided = 1, kPathSymmetric = 2 };
-constexpr int64_t kSymMinN = 8192;                // auto: symmetric kernel from here on.  The kernel alone wins from ~6,000
-                                                  // elements, but its 126 registers leave the contact pass no room to run
-                                                  // beside it; measured whole steps (one-sided / symmetric, us): 8,192: 64 / 67,
-                                                  // 10,240: 79 / 78, 12,288: 105 / 89, 16,384: 164 / 137, 24,576: 331 / 243
+constexpr int64_t kSymMinN = 8192;                // auto: symmetric kernel from here on (below: the fused one-launch kernel).
+                                                  // Measured whole steps, one-sided / symmetric, us (profiles/r2_crossover.md):
+                                                  // 8,192: 74 / 60, 10,240: 84 / 70, 12,288: 109 / 89, 16,384: 158 / 131,
+                                                  // 24,576: 328 / 252
 constexpr int64_t kSym256MaxN = 32768;             // below this the super-tiles are 256 elements (CTAs of 2 warps)
 constexpr int64_t kSymMaxN = (int64_t)1 << 26;    // ... for every n the library takes
 constexpr int64_t kChainMinN = 98304;             // from here on (S >= 1,024) the symmetric kernel runs in chain mode: its T
