@@ -59,7 +59,8 @@ typedef enum {
     NB_ESTATE = -2,   /* call order (no state set), or star[] not 0...0 1...1 */
     NB_ECUDA = -3,    /* a CUDA call failed; see nb_last_cuda_error() */
     NB_ENOMEM = -4,   /* workspace too small / host allocation failed */
-    NB_EARCH = -5     /* the current device is not sm_100 */
+    NB_EARCH = -5,    /* the current device is not sm_100 */
+    NB_ESIZE = -6     /* n exceeds the fixed scratch of nb_gravity_accel_static() (see its limit) */
 } nb_status;
 
 typedef struct {
@@ -213,6 +214,48 @@ int nb_time_contact_pass(nb_ctx* ctx, int reps, float* ms_avg);
  * unordered contacts).  n < 8192 (no cell list): out2[0] = n (n - 1), out2[1] = -1.  gamma == 0: zeros.
  * The partial sums it writes touch no state.  Synchronises the stream. */
 int nb_contact_stats(nb_ctx* ctx, int64_t* out2);
+
+/* ---- Gravity accelerations for callers that cannot allocate device memory ------------------------------
+ *
+ * Everything above needs a workspace the caller has to get from somewhere (3 MiB at n = 2048), plus a ctx
+ * whose creation makes a stream and two events.  Some users of this library have no way to obtain that
+ * memory: code loaded as a plug-in into a host application that hands it exactly the state arrays and keeps
+ * its allocator to itself, code running under a fixed, fully assigned memory budget, and code inside a
+ * latency-critical loop where cudaMalloc/cudaFree are off limits because they stall the whole device.
+ * For them this one call evaluates row a2 -- Eq. 4 summed over all pairs,
+ *   a_i = sum_{j != i} G m_j d / (r (r + eps)^2),  d = x_j - x_i,  r = |d|  (coincident pairs add nothing) --
+ * with the one-sided all-pairs kernel (NB_PATH_ONE_SIDED above) and needs nothing but its inputs and its
+ * output: the kernel's scratch (the partial sums of its j splits, which a second kernel adds up in split
+ * order) lives in a fixed array inside the library image instead of a workspace.  No ctx, no contact terms
+ * (gamma = 0), no stepping.
+ *
+ *   posm: dev float[n][4] (x, y, z, m), 16-byte aligned, read only.   acc: dev float[n][4], 16-byte aligned,
+ *   receives (ax, ay, az, 0); must not overlap posm.   cuda_stream: cudaStream_t (NULL = legacy default
+ *   stream); the two launches are asynchronous on it.   cuda_error: HOST, may be NULL; receives the
+ *   cudaError_t when the call returns NB_ECUDA, else 0.
+ *
+ * Limit: 1 <= n <= nb_gravity_accel_static_max_n() = 16384.  A larger n returns NB_ESIZE and launches
+ * nothing -- use the ctx API with a caller-provided workspace there.
+ *
+ * Costs and rules that follow from the fixed array:
+ *   - it is 2 MiB (131072 float4) of device memory on EVERY GPU this process uses the library on, held
+ *     from the moment the library is loaded there until the process exits, whether or not this is called;
+ *   - the call itself performs no cudaMalloc, no cudaFree, creates no stream or event and calls no library
+ *     routine that allocates;
+ *   - the first call on a device looks up the array's device address (once per device, with that device
+ *     current) and the device's SM count and compute capability; later calls on that device reuse them.
+ *     Make that first call before you begin any stream capture;
+ *   - every call on a device uses the same array, and it still holds the previous call's partial sums
+ *     when the next one starts.  Nothing has to be zeroed: each call writes every slot before it reads it.
+ *     But two calls whose kernels are in flight on the same device at once (different streams, or
+ *     different host threads) overwrite each other's partial sums -- the results of both are garbage and
+ *     nothing reports it.  Keep all calls on one device on one stream, or order them with events.
+ * Returns NB_EINVAL (null/misaligned pointer, n < 1, G or eps negative or not finite), NB_ESIZE, NB_EARCH
+ * (device is not sm_100), NB_ECUDA, else NB_OK.  Thread-safe as far as the set-up goes (a mutex guards the
+ * per-device table); the sharing rule above still applies. */
+int nb_gravity_accel_static(int64_t n, const float* posm, float G, float eps, float* acc, void* cuda_stream,
+                            int* cuda_error);
+int64_t nb_gravity_accel_static_max_n(void);
 
 void nb_destroy(nb_ctx* ctx);
 const char* nb_strerror(int status);

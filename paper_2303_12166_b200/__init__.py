@@ -15,7 +15,7 @@ from typing import Dict, Optional, Sequence
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("NB_LIB_PATH") or os.path.join(HERE, "libnb.so")   # override: development only
 
-NB_OK, NB_EINVAL, NB_ESTATE, NB_ECUDA, NB_ENOMEM, NB_EARCH = 0, -1, -2, -3, -4, -5
+NB_OK, NB_EINVAL, NB_ESTATE, NB_ECUDA, NB_ENOMEM, NB_EARCH, NB_ESIZE = 0, -1, -2, -3, -4, -5, -6
 NB_PATH_AUTO, NB_PATH_ONE_SIDED, NB_PATH_SYMMETRIC = 0, 1, 2
 
 EXPORTS = ("nb_create", "nb_workspace_bytes", "nb_set_state", "nb_compute_accel", "nb_step",
@@ -23,7 +23,8 @@ EXPORTS = ("nb_create", "nb_workspace_bytes", "nb_set_state", "nb_compute_accel"
            "nb_download_state",
            "nb_get_launch_info", "nb_set_force_path", "nb_force_kernel_name", "nb_launch_count",
            "nb_time_force_kernel", "nb_time_contact_pass", "nb_contact_stats", "nb_destroy", "nb_strerror",
-           "nb_last_cuda_error", "nb_roche_lobe_radius", "nb_l1_distance")
+           "nb_last_cuda_error", "nb_roche_lobe_radius", "nb_l1_distance",
+           "nb_gravity_accel_static", "nb_gravity_accel_static_max_n")
 
 
 class nb_params(C.Structure):
@@ -106,6 +107,10 @@ def lib() -> C.CDLL:
         L.nb_roche_lobe_radius.argtypes = [C.c_double, C.c_double]
         L.nb_l1_distance.restype = C.c_double
         L.nb_l1_distance.argtypes = [C.c_double]
+        L.nb_gravity_accel_static.restype = C.c_int
+        L.nb_gravity_accel_static.argtypes = [i64, vp, C.c_float, C.c_float, vp, vp, C.POINTER(C.c_int)]
+        L.nb_gravity_accel_static_max_n.restype = i64
+        L.nb_gravity_accel_static_max_n.argtypes = []
         _lib = L
     return _lib
 
@@ -279,6 +284,24 @@ def nb_roche_lobe_radius(mass_ratio: float, k: float = 0.6) -> float:
 
 def nb_l1_distance(q: float) -> float:
     return float(lib().nb_l1_distance(float(q)))
+
+
+def nb_gravity_accel_static_max_n() -> int:
+    return int(lib().nb_gravity_accel_static_max_n())
+
+
+def nb_gravity_accel_static(n: int, posm, G: float, eps: float, acc, cuda_stream: int = 0) -> None:
+    """Eq. 4 accelerations of n <= nb_gravity_accel_static_max_n() elements into `acc` with no workspace and no ctx:
+    for callers that cannot get device memory of their own (a plug-in inside a host application that owns the
+    allocator, a fixed memory budget, a loop where cudaMalloc's device-wide stall is not acceptable).  The kernel's
+    partial sums go to a 2 MiB array built into libnb.so, one per device and shared by every call on it: calls that
+    overlap on a device corrupt each other, so keep them on one stream.  Make the first call on a device before any
+    stream capture.  `posm`, `acc`: device float32 [n][4].  Raises NbError (NB_ESIZE beyond the limit)."""
+    err = C.c_int(0)
+    rc = lib().nb_gravity_accel_static(int(n), _ptr(posm), float(G), float(eps), _ptr(acc), C.c_void_p(cuda_stream or None),
+                                       C.byref(err))
+    if rc != NB_OK:
+        raise NbError(rc, "nb_gravity_accel_static", err.value)
 
 
 class Simulation:

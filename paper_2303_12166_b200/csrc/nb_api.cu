@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 using namespace nb;
@@ -555,6 +556,7 @@ const char* nb_strerror(int status)
         case NB_ECUDA: return "CUDA error (see nb_last_cuda_error)";
         case NB_ENOMEM: return "workspace too small or host allocation failed";
         case NB_EARCH: return "device is not sm_100 (B200)";
+        case NB_ESIZE: return "n exceeds nb_gravity_accel_static_max_n(): the entry point without a workspace has a fixed scratch array; use the ctx API";
         default: return "unknown status";
     }
 }
@@ -1073,6 +1075,100 @@ double nb_l1_distance(double q)
         s = sn;
     }
     return s;
+}
+
+
+// ---------------------------------------------------------------------------------------------------------
+// nb_gravity_accel_static(): row a2 (Eq. 4, summed over all pairs) for callers
+// that have no way to get device memory for a workspace -- see include/nb.h for who they are.  The
+// one-sided gravity kernel needs scratch: a CTA owns an (i-block, j-split) and writes the partial
+// acceleration of its elements i due to its split of the elements j into slab `split` of n float4;
+// nb_reduce_update_kernel then adds the slabs of an element in split order.  Everywhere else those slabs sit
+// in the caller's workspace; here they sit in the array below, which is part of the library image: the
+// driver places it on every device that loads this module and keeps it there until the process ends.
+namespace {
+
+constexpr int64_t kStaticMaxN = 16384;                       // largest n the entry point takes
+constexpr int64_t kStaticSlots = 8 * kStaticMaxN;            // float4 partial sums: 2 MiB; n * splits <= this
+constexpr int kStaticMaxDevices = 64;
+
+static __device__ __align__(256) float4 nb_static_scratch[kStaticSlots];
+
+// In host code `nb_static_scratch` is only a handle for the runtime's symbol calls -- it is NOT the array's
+// device address, and a kernel handed `nb_static_scratch` from the host side would write somewhere else or
+// fault.  The address a kernel can use comes from cudaGetSymbolAddress(), differs from device to device,
+// and is looked up once per device (with that device current) and kept here.
+struct StaticDevice {
+    float4* scratch = nullptr;
+    int num_sms = 0;
+    bool ready = false;
+};
+StaticDevice g_static_device[kStaticMaxDevices];
+std::mutex g_static_mutex;
+
+// Per-device set-up of the first call on the current device.  Allocates nothing.
+int static_device(const StaticDevice** out, cudaError_t* err)
+{
+    int dev = -1;
+    if ((*err = cudaGetDevice(&dev)) != cudaSuccess) return NB_ECUDA;
+    if (dev < 0 || dev >= kStaticMaxDevices) return NB_EINVAL;
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    StaticDevice& d = g_static_device[dev];
+    if (!d.ready) {
+        int major = 0, sms = 0;
+        if ((*err = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev)) != cudaSuccess) return NB_ECUDA;
+        if (major != 10) return NB_EARCH;
+        if ((*err = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev)) != cudaSuccess) return NB_ECUDA;
+        float4* ptr = nullptr;
+        if ((*err = cudaGetSymbolAddress((void**)&ptr, nb_static_scratch)) != cudaSuccess) return NB_ECUDA;
+        if (!ptr) { *err = cudaErrorInvalidSymbol; return NB_ECUDA; }
+        d.scratch = ptr;
+        d.num_sms = sms > 0 ? sms : kNumSMsFallback;
+        d.ready = true;
+    }
+    *out = &d;
+    return NB_OK;
+}
+
+}  // namespace
+
+int64_t nb_gravity_accel_static_max_n(void) { return kStaticMaxN; }
+
+int nb_gravity_accel_static(int64_t n, const float* posm, float G, float eps, float* acc, void* cuda_stream, int* cuda_error)
+{
+    if (cuda_error) *cuda_error = 0;
+    if (!posm || !acc || n < 1) return NB_EINVAL;
+    if (n > kStaticMaxN) return NB_ESIZE;                    // before anything touches the device
+    if ((reinterpret_cast<uintptr_t>(posm) | reinterpret_cast<uintptr_t>(acc)) & 15u) return NB_EINVAL;
+    if (!std::isfinite(G) || !std::isfinite(eps) || G < 0.f || eps < 0.f) return NB_EINVAL;
+    cudaError_t err = cudaSuccess;
+    auto fail = [&](int rc) { if (cuda_error) *cuda_error = (int)err; return rc; };
+    const StaticDevice* d = nullptr;
+    if (int rc = static_device(&d, &err)) return fail(rc);
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+
+    // the one-sided plan of the ctx API, with its j splits cut to what the fixed array holds
+    Plan p = make_plan(n, d->num_sms, kPathOneSided);
+    const int64_t room = kStaticSlots / n;                   // >= 8
+    if (p.nsplit > room) p.nsplit = (int)room;
+    if (p.nsplit > p.njt) p.nsplit = p.njt;                  // every split holds at least one tile
+    GravArgs ga;
+    ga.posm = reinterpret_cast<const float4*>(posm); ga.part = d->scratch;
+    ga.n = (int)n; ga.nib = p.nib; ga.nsplit = p.nsplit; ga.njt = p.njt;
+    ga.G = G; ga.eps = eps;
+    const int grid = p.nib * p.nsplit;
+    // every slot [split][i], i < n, split < nsplit, is written here before the reduction reads it: whatever an
+    // earlier call left in the array is never seen
+    if (p.TJ == 256) nb_gravity_kernel<2, 256><<<grid, kThreads, 0, st>>>(ga);
+    else             nb_gravity_kernel<2, 128><<<grid, kThreads, 0, st>>>(ga);
+    if ((err = cudaGetLastError()) != cudaSuccess) return fail(NB_ECUDA);
+    UpdateArgs u;
+    u.acc64 = nullptr; u.src = d->scratch; u.acc_out = reinterpret_cast<float4*>(acc);
+    u.posm = nullptr; u.vel = nullptr; u.dev = nullptr;      // no kick, no drift, no step count: untouched
+    u.n = (int)n; u.nsrc = p.nsplit; u.kick_h = 0.f; u.drift_dt = 0.f; u.vscale = 1.f; u.advance = 0;
+    nb_reduce_update_kernel<<<(int)((n + 255) / 256), 256, 0, st>>>(u);
+    if ((err = cudaGetLastError()) != cudaSuccess) return fail(NB_ECUDA);
+    return NB_OK;
 }
 
 }  // extern "C"
