@@ -14,7 +14,8 @@
  *     or throws.  nb_strerror() gives the text; for NB_ECUDA, nb_last_cuda_error()
  *     gives the cudaError_t.
  *   - "dev" pointers are CUDA device pointers on the device that was current
- *     at nb_create(); "host" pointers are ordinary host memory.
+ *     at nb_create(); "host" pointers are ordinary host memory.  That device must
+ *     be current in every later call on the ctx (NB_ESTATE otherwise).
  *   - The CALLER owns every device byte (state, output, workspace).  The
  *     library owns only the host-side nb_ctx (plus one internal stream and two events: SURVEY 8(b) says
  *     "owns only the host-side nb_ctx" -- the stream carries the contact pass beside the gravity kernel and
@@ -148,8 +149,11 @@ int nb_get_step(nb_ctx* ctx, int64_t* step, float* R);
 /* Restore the step count n of a checkpointed run (the element radius is a function of
  * how far the run has come): sets n = step and R_s(n) by the expanding-star rule, exactly as nsteps
  * calls of nb_step() from 0 would have left them.  The full state of a run is (x, v, a(x_n), n):
- * nb_upload_state() restores the arrays, this call the count.  The cached acceleration is kept (it
- * belongs to the uploaded state).  step >= 0.  Asynchronous on the stream. */
+ * nb_upload_state() restores the arrays, this call the count.  A cached acceleration that came with
+ * nb_upload_state(host_acc) is kept (it belongs to the uploaded state: upload first, then set the step).
+ * One evaluated by this ctx (nb_compute_accel, nb_step, ...) holds contact terms at the OLD radii: it is
+ * dropped when the radii move with the step count (gamma > 0, n_ramp > 0, R_start != R_end), and the next
+ * step evaluates a(x) again at R_s(step).  step >= 0.  Asynchronous on the stream. */
 int nb_set_step(nb_ctx* ctx, int64_t step);
 
 /* Host-buffer entry points for end-to-end use and checkpoint/restart: copy HOST
@@ -188,8 +192,9 @@ int nb_get_launch_info(nb_ctx* ctx, int32_t* out4);
  * For n >= 98304 the symmetric kernel runs in "chain mode": its CTAs add their results into one pair of fp64 sums per
  * element, super-tile by super-tile in a fixed order kept by turn counters (still bitwise reproducible, no atomics
  * on data).  Should a turn ever fail to come (it cannot by construction; the check keeps a bug from hanging the GPU),
- * the next synchronising call (nb_energy, nb_get_step, nb_download_state) returns NB_ECUDA with
- * nb_last_cuda_error() == cudaErrorLaunchTimeout. */
+ * an error word is raised on the device that only nb_set_state() clears: every synchronising call from then on
+ * (nb_energy, nb_get_step, nb_download_state) returns NB_ECUDA with nb_last_cuda_error() == cudaErrorLaunchTimeout
+ * and drops the cached acceleration -- the state has been stepped with sums added out of order; rebind it. */
 enum { NB_PATH_AUTO = 0, NB_PATH_ONE_SIDED = 1, NB_PATH_SYMMETRIC = 2 };
 int nb_set_force_path(nb_ctx* ctx, int path);
 
@@ -204,7 +209,9 @@ int64_t nb_launch_count(nb_ctx* ctx);
  * pairs; nb_time_force_kernel) or the contact pass (row a3: cell list -- bbox, count, scan, scatter, rank -- and Eqs. 5/6;
  * nb_time_contact_pass, 0 ms when gamma == 0) `reps` times on the ctx stream after one warm-up,
  * bracketed by CUDA events on that stream; HOST *ms_avg receives the average duration of one
- * pass.  Their partial sums land in the workspace and touch no state.  Synchronise the stream. */
+ * pass.  Their partial sums land in the workspace and touch no state (in chain mode, n >= 98304, the
+ * gravity launches overwrite the fp64 accumulators of the last force evaluation -- the cached acceleration
+ * is a separate array and stays valid -- and leave the chain error word alone).  Synchronise the stream. */
 int nb_time_force_kernel(nb_ctx* ctx, int reps, float* ms_avg);
 int nb_time_contact_pass(nb_ctx* ctx, int reps, float* ms_avg);
 

@@ -37,8 +37,10 @@ struct Plan {           // launch configuration of the gravity kernel for a give
 constexpr int kCtasPerSM = 8;                      // resident CTAs/SM of nb_gravity_kernel<2, .> (64 registers)
 constexpr int64_t kMaxSplit = 64;
 constexpr int64_t kPartialBudget = (int64_t)128 << 20;   // bytes of split-j partial sums worth keeping in L2
-constexpr int64_t kCellMinN = 8192;                // below this the contact pass takes groups in index order (all pairs
-                                                   // pre-tested), from here on it builds the cell list
+constexpr int64_t kCellMinN = 8192;                // from here on the contact pass builds the cell list.  Below, contact terms are
+                                                   // found inside nb_fused_step_kernel's all-pairs loop; the separate index-order
+                                                   // pass (all pairs pre-tested) runs only when that kernel is unavailable or a
+                                                   // path is forced, and under nb_time_contact_pass / nb_contact_stats
 constexpr int64_t kContactWideN = 131072;          // cell list: below this, 4 lanes share the rows of an element's query
                                                    // (measured: 16,384: 45 vs 67 us per pass, 65,536: 50 vs 53; 262,144: 129 vs 107)
 constexpr int kMaxContactChunks = 32;              // index-order search: the candidate groups of a warp go to this many slabs
@@ -134,7 +136,8 @@ Plan make_plan(int64_t n, int num_sms, int path)
     p.njt = (int)((n + p.TJ - 1) / p.TJ);
     const int64_t slots = (int64_t)num_sms * kCtasPerSM;
     int64_t pmax = p.njt >= 2 ? p.njt / 2 : 1;
-    if (n < kCellMinN) pmax = p.njt;                 // small n (the unfused path: nb_relax, no cooperative launch): down to one tile per CTA
+    if (n < kCellMinN) pmax = p.njt;                 // small n, reached only without the fused kernel (no cooperative launch) and by
+                                                     // nb_gravity_accel_static / nb_time_force_kernel: down to one tile per CTA
     if (pmax > max_split(n)) pmax = max_split(n);
     double best = 0.0;
     for (int64_t P = 1; P <= pmax; ++P) {
@@ -202,6 +205,7 @@ struct nb_ctx {
     cudaStream_t side = nullptr;          // library-owned: the contact pass runs here, beside the gravity kernel
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int num_sms = kNumSMsFallback;
+    int device = -1;                      // the device that was current at nb_create(): every pointer and kernel attribute belongs to it
     bool fused_ok = false;                // cooperative launch + the shared memory of nb_fused_step_kernel are available
     int fused_blocks = 0, fused_logP = 0; // CTAs of nb_fused_step_kernel for the bound state (0: not available) and its 2^logP pairs per CTA
     float4* posm = nullptr;
@@ -210,6 +214,7 @@ struct nb_ctx {
     Layout lay{};
     Plan plan{};
     bool have_state = false, have_acc = false;
+    bool acc_uploaded = false;            // the cached a(x) came from nb_upload_state(host_acc), not from a force evaluation here
     bool chain_launched = false;          // the turn counters / error flag of chain mode hold a launch's state
     int path = kPathAuto;
     int last_cuda = 0;
@@ -246,6 +251,15 @@ struct nb_ctx {
 
 namespace {
 
+// Every entry point that touches the device runs with the ctx's device current (nb.h: "dev" pointers belong to the
+// device that was current at nb_create(), and so do the kernels' shared-memory opt-ins).
+int device_guard(nb_ctx* c)
+{
+    int dev = -1;
+    NB_CUDA(c, cudaGetDevice(&dev));
+    return dev == c->device ? NB_OK : NB_ESTATE;
+}
+
 bool params_ok(const nb_params* p)
 {
     auto fin = [](float x) { return std::isfinite(x); };
@@ -281,26 +295,18 @@ int launch_sym(nb_ctx* c, SymArgs& sa, int grid)
     using K = SymShape<S>;
     const int smem = kSymSmemPerElem * S;
     if (c->plan.chain) {                              // nb_kernels.cuh "Chain mode"
-        auto kernel = nb_gravity_sym_chain_kernel<S, K::NI, K::NT, K::MINB, K::UNR>;
-        static bool configured = false;
-        if (!configured) {
-            NB_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-            configured = true;
-        }
+        auto kernel = nb_gravity_sym_chain_kernel<S, K::NI, K::NT, K::MINB, K::UNR>;   // shared-memory opt-in: configure_kernels()
         sa.acc64 = c->template at<double>(c->lay.off_acc64);
         sa.turn = c->template at<int>(c->lay.off_turn);
         constexpr int kRounds = S / (K::NT * K::NI);
-        NB_CUDA(c, cudaMemsetAsync(sa.turn, 0, ((size_t)sa.T * (kRounds + 1) + 2) * sizeof(int), c->stream));
+        // turn counters and the ticket start at zero; the error word behind them is NOT cleared here: it is sticky from
+        // nb_set_state() on, so a turn lost at step k of nb_step(100) is still there when the caller synchronises
+        NB_CUDA(c, cudaMemsetAsync(sa.turn, 0, ((size_t)sa.T * (kRounds + 1) + 1) * sizeof(int), c->stream));
         kernel<<<grid, K::NT, smem, c->stream>>>(sa);
         c->chain_launched = true;
         return NB_OK;
     }
-    auto kernel = nb_gravity_sym_kernel<S, K::NI, K::NT, K::MINB, K::UNR>;
-    static bool configured = false;                   // the kernel's shared memory is dynamic (112 KB at S = 4096)
-    if (!configured) {
-        NB_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        configured = true;
-    }
+    auto kernel = nb_gravity_sym_kernel<S, K::NI, K::NT, K::MINB, K::UNR>;   // dynamic shared memory (112 KB at S = 4096)
     kernel<<<grid, K::NT, smem, c->stream>>>(sa);
     return NB_OK;
 }
@@ -313,6 +319,35 @@ const char* sym_name(bool chain)
     std::snprintf(buf[chain], sizeof(buf[chain]), "nb_gravity_sym_%skernel<%d,%d,%d,%d,%d>", chain ? "chain_" : "", S, K::NI, K::NT,
                   K::MINB, K::UNR);
     return buf[chain];
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a property of (kernel, DEVICE): every kernel that takes more than
+// 48 KB of dynamic shared memory is opted in on the current device by nb_create(), once per ctx (a few host-side
+// calls), not once per process -- a ctx created on a second GPU of the same process needs its own opt-in.
+template <int S>
+cudaError_t configure_sym()
+{
+    using K = SymShape<S>;
+    const int smem = kSymSmemPerElem * S;
+    cudaError_t e = cudaFuncSetAttribute(nb_gravity_sym_kernel<S, K::NI, K::NT, K::MINB, K::UNR>,
+                                         cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    if (e != cudaSuccess) return e;
+    if (S >= 1024)
+        e = cudaFuncSetAttribute(nb_gravity_sym_chain_kernel<S, K::NI, K::NT, K::MINB, K::UNR>,
+                                 cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    return e;
+}
+
+cudaError_t configure_kernels()
+{
+    cudaError_t e;
+    if ((e = configure_sym<256>()) != cudaSuccess) return e;
+    if ((e = configure_sym<512>()) != cudaSuccess) return e;
+    if ((e = configure_sym<1024>()) != cudaSuccess) return e;
+    if ((e = configure_sym<2048>()) != cudaSuccess) return e;
+    if ((e = configure_sym<4096>()) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(nb_pot_pair_kernel<4096, 8, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 4096)) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(nb_pot_pair_kernel<8192, 8, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 8192);
 }
 
 // Row a2: partial gravitational accelerations -> part[0..ngrav-1][n]
@@ -522,7 +557,11 @@ int chain_flag_check(nb_ctx* c)
     NB_CUDA(c, cudaMemcpyAsync(&flag, c->at<int>(c->lay.off_turn) + (size_t)c->plan.T * (rounds + 1) + 1, sizeof(int),
                                cudaMemcpyDeviceToHost, c->stream));
     NB_CUDA(c, cudaStreamSynchronize(c->stream));
-    if (flag) { c->last_cuda = (int)cudaErrorLaunchTimeout; return NB_ECUDA; }
+    if (flag) {                                          // sums added out of turn: a(x) and everything stepped with it is void
+        c->have_acc = false;
+        c->last_cuda = (int)cudaErrorLaunchTimeout;
+        return NB_ECUDA;
+    }
     return NB_OK;
 }
 
@@ -532,14 +571,14 @@ int ensure_acc(nb_ctx* c)
     if (fused_path(c)) {
         const int rc = launch_fused(c, 1, 0, 1, nullptr);
         if (rc) return rc;
-        c->have_acc = true;
+        c->have_acc = true; c->acc_uploaded = false;
         return NB_OK;
     }
     int rc = launch_force(c);
     if (rc) return rc;
     rc = launch_update(c, c->part(), c->nslabs(), c->acc(), 0.f, 0.f, 0);
     if (rc) return rc;
-    c->have_acc = true;
+    c->have_acc = true; c->acc_uploaded = false;
     return NB_OK;
 }
 
@@ -585,7 +624,12 @@ int nb_create(nb_ctx** out, int64_t n_max, const nb_params* p, void* cuda_stream
     c->n_max = n_max;
     c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
     c->num_sms = sms > 0 ? sms : kNumSMsFallback;
+    c->device = dev;
     c->lay = make_layout(n_max);
+    {
+        const cudaError_t e = configure_kernels();
+        if (e != cudaSuccess) { cudaGetLastError(); delete c; return NB_ECUDA; }
+    }
     // default priority, like the gravity kernel launched before it: see launch_force()
     if (cudaStreamCreateWithFlags(&c->side, cudaStreamNonBlocking) != cudaSuccess ||
         cudaEventCreateWithFlags(&c->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
@@ -622,8 +666,10 @@ int nb_set_state(nb_ctx* c, int64_t n, float* posm, float* vel, const int32_t* s
         ((uintptr_t)workspace & (kAlign - 1)))
         return NB_EINVAL;
     if (workspace_bytes < c->lay.total) return NB_ENOMEM;
+    if (int rc_ = device_guard(c)) return rc_;
     c->have_state = false;
     c->have_acc = false;
+    c->acc_uploaded = false;
     c->chain_launched = false;
     c->ws = static_cast<char*>(workspace);
 
@@ -642,6 +688,10 @@ int nb_set_state(nb_ctx* c, int64_t n, float* posm, float* vel, const int32_t* s
     NB_CUDA(c, cudaMemcpyAsync(&h, c->dev(), sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     NB_CUDA(c, cudaStreamSynchronize(c->stream));
     if (h.bad) return NB_ESTATE;
+    // chain mode's turn counters, ticket and ERROR WORD: all zero from here on; the launches clear the counters and the
+    // ticket again, nothing but this call clears the error word (its position depends on n only)
+    if (c->n_max >= kChainMinN)
+        NB_CUDA(c, cudaMemsetAsync(c->at<int>(c->lay.off_turn), 0, ((size_t)(c->n_max / 1024 + 1) * 5 + 2) * sizeof(int), c->stream));
 
     c->n = n;
     c->n1 = h.n1;
@@ -658,10 +708,11 @@ int nb_compute_accel(nb_ctx* c, float* acc)
 {
     if (!c || !acc || ((uintptr_t)acc & 15)) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
     if (fused_path(c)) {
         const int rc = launch_fused(c, 1, 0, 1, reinterpret_cast<float4*>(acc) != c->acc() ? reinterpret_cast<float4*>(acc) : nullptr);
         if (rc) return rc;
-        c->have_acc = true;
+        c->have_acc = true; c->acc_uploaded = false;
         return NB_OK;
     }
     int rc = launch_force(c);
@@ -672,7 +723,7 @@ int nb_compute_accel(nb_ctx* c, float* acc)
         NB_CUDA(c, cudaMemcpyAsync(c->acc(), acc, (size_t)c->n * sizeof(float4), cudaMemcpyDeviceToDevice,
                                    c->stream));
     }
-    c->have_acc = true;
+    c->have_acc = true; c->acc_uploaded = false;
     return NB_OK;
 }
 
@@ -680,6 +731,7 @@ int nb_step(nb_ctx* c, int nsteps)
 {
     if (!c || nsteps < 0) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
     if (nsteps == 0) return NB_OK;
     const float dt = c->prm.dt;
     int rc = ensure_acc(c);                                    // a(x_n) with v_n (A7)
@@ -697,7 +749,7 @@ int nb_step(nb_ctx* c, int nsteps)
             rc = launch_update(c, c->part(), c->nslabs(), c->acc(), 0.5f * dt, 0.f, 0);
         if (rc) return rc;
     }
-    c->have_acc = true;
+    c->have_acc = true; c->acc_uploaded = false;
     return NB_OK;
 }
 
@@ -705,6 +757,7 @@ int nb_relax(nb_ctx* c, int nsteps, float kappa)
 {
     if (!c || nsteps < 0 || !(kappa >= 0.f) || !std::isfinite(kappa)) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
     if (nsteps == 0) return NB_OK;
     const float dt = c->prm.dt;
     float f = 1.f - kappa * dt;                               // rounded as written: one multiply, one subtract
@@ -720,7 +773,7 @@ int nb_relax(nb_ctx* c, int nsteps, float kappa)
         rc = launch_update(c, c->part(), c->nslabs(), c->acc(), 0.5f * dt, 0.f, 0, f);   // half kick, then v <- f v
         if (rc) return rc;
     }
-    c->have_acc = true;
+    c->have_acc = true; c->acc_uploaded = false;
     return NB_OK;
 }
 
@@ -728,6 +781,7 @@ int nb_transfer_diagnostics(nb_ctx* c, double k_lobe, double* out)
 {
     if (!c || !out || !(k_lobe > 0.0) || !std::isfinite(k_lobe)) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
     const int n = (int)c->n;
     double* red = c->red();
     double h1[kMomentBlocks * kXferCols1], h2[kMomentBlocks * kXferCols2];
@@ -785,6 +839,7 @@ int nb_splat(nb_ctx* c, const float* centre, float half_width, int axis_u, int a
     if (axis_u < 0 || axis_u > 2 || axis_v < 0 || axis_v > 2 || axis_u == axis_v) return NB_EINVAL;
     if (W < 1 || H < 1 || W > 16384 || H > 16384 || ((uintptr_t)image & 3)) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
     const float scale = (float)W / (2.0f * half_width);        // pixels per unit length, fp32
     NB_CUDA(c, cudaMemsetAsync(image, 0, (size_t)2 * W * H * sizeof(uint32_t), c->stream));
     nb_splat_kernel<<<(int)((c->n + 255) / 256), 256, 0, c->stream>>>(c->posm, (int)c->n, c->n1, centre[axis_u],
@@ -798,6 +853,7 @@ int nb_get_step(nb_ctx* c, int64_t* step, float* R)
 {
     if (!c) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
     DevState h;
     NB_CUDA(c, cudaMemcpyAsync(&h, c->dev(), sizeof(h), cudaMemcpyDeviceToHost, c->stream));
     NB_CUDA(c, cudaStreamSynchronize(c->stream));
@@ -811,9 +867,15 @@ int nb_set_step(nb_ctx* c, int64_t step)
 {
     if (!c || step < 0) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
     nb_set_step_kernel<<<1, 1, 0, c->stream>>>(c->dev(), (long long)step);
     c->launches++;
     NB_CUDA(c, cudaGetLastError());
+    // A cached a(x) holds contact terms at the radii of the step it was evaluated at.  It stays only when it cannot be
+    // stale: the radii do not move with the step count, or it was uploaded with the checkpoint this call completes.
+    const bool radii_move = c->contact_on() && c->prm.n_ramp > 0 &&
+                            (c->prm.R_start[0] != c->prm.R_end[0] || c->prm.R_start[1] != c->prm.R_end[1]);
+    if (radii_move && !c->acc_uploaded) c->have_acc = false;
     return NB_OK;
 }
 
@@ -821,6 +883,7 @@ int nb_energy(nb_ctx* c, double* out)
 {
     if (!c || !out) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
     int rc = ensure_acc(c);
     if (rc) return rc;
     rc = chain_flag_check(c);
@@ -856,15 +919,8 @@ int nb_energy(nb_ctx* c, double* out)
         nb_tile_bbox_kernel<<<pa.T, 256, 0, c->stream>>>(pa.px, n, S, tbox);
         c->launches++;
         if (S == 1024)      nb_pot_pair_kernel<1024, 8, 128><<<(unsigned)npot, 128, 16 * 1024, c->stream>>>(pa);
-        else if (S == 4096) {
-            static bool cfg = false;
-            if (!cfg) { NB_CUDA(c, cudaFuncSetAttribute(nb_pot_pair_kernel<4096, 8, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 4096)); cfg = true; }
-            nb_pot_pair_kernel<4096, 8, 128><<<(unsigned)npot, 128, 16 * 4096, c->stream>>>(pa);
-        } else {
-            static bool cfg = false;
-            if (!cfg) { NB_CUDA(c, cudaFuncSetAttribute(nb_pot_pair_kernel<8192, 8, 128>, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 8192)); cfg = true; }
-            nb_pot_pair_kernel<8192, 8, 128><<<(unsigned)npot, 128, 16 * 8192, c->stream>>>(pa);
-        }
+        else if (S == 4096) nb_pot_pair_kernel<4096, 8, 128><<<(unsigned)npot, 128, 16 * 4096, c->stream>>>(pa);   // > 48 KB: configure_kernels()
+        else                nb_pot_pair_kernel<8192, 8, 128><<<(unsigned)npot, 128, 16 * 8192, c->stream>>>(pa);
         c->launches++;
         NB_CUDA(c, cudaGetLastError());
     } else {
@@ -914,11 +970,13 @@ int nb_upload_state(nb_ctx* c, const float* host_posm, const float* host_vel, co
 {
     if (!c) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
     const size_t bytes = (size_t)c->n * sizeof(float4);
     if (host_posm) NB_CUDA(c, cudaMemcpyAsync(c->posm, host_posm, bytes, cudaMemcpyHostToDevice, c->stream));
     if (host_vel) NB_CUDA(c, cudaMemcpyAsync(c->vel, host_vel, bytes, cudaMemcpyHostToDevice, c->stream));
     if (host_acc) NB_CUDA(c, cudaMemcpyAsync(c->acc(), host_acc, bytes, cudaMemcpyHostToDevice, c->stream));
     c->have_acc = host_acc != nullptr;
+    c->acc_uploaded = c->have_acc;
     return NB_OK;
 }
 
@@ -926,6 +984,7 @@ int nb_download_state(nb_ctx* c, float* host_posm, float* host_vel, float* host_
 {
     if (!c) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
     const size_t bytes = (size_t)c->n * sizeof(float4);
     if (host_acc) {
         const int rc = ensure_acc(c);
@@ -942,6 +1001,7 @@ int nb_get_launch_info(nb_ctx* c, int32_t* out4)
 {
     if (!c || !out4) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
     if (fused_path(c)) {                  // one cooperative launch: elements i per CTA, j segments per CTA, CTAs
         out4[0] = 2 << c->fused_logP;
         out4[1] = kFusedThreads >> c->fused_logP;
@@ -993,6 +1053,7 @@ int time_launches(nb_ctx* c, int reps, float* ms_avg, int (*launch)(nb_ctx*))
 {
     if (!c || !ms_avg || reps < 1) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
     cudaEvent_t e0, e1;
     NB_CUDA(c, cudaEventCreate(&e0));
     NB_CUDA(c, cudaEventCreate(&e1));
@@ -1018,6 +1079,7 @@ int nb_contact_stats(nb_ctx* c, int64_t* out2)
 {
     if (!c || !out2) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
     out2[0] = out2[1] = 0;
     if (!c->contact_on()) return NB_OK;
     if (c->n < kCellMinN) {                                    // no cell list: every ordered pair is pre-tested
