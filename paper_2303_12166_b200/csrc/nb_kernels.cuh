@@ -931,7 +931,7 @@ __device__ __forceinline__ double contact_potential(const ContactArgs& a, const 
     const double dx = (double)pj.x - (double)pi.x, dy = (double)pj.y - (double)pi.y, dz = (double)pj.z - (double)pi.z;
     const double r2 = dx * dx + dy * dy + dz * dz;
     const double D = (double)pi.w + (double)pj.w;
-    if (!(r2 < D * D) || r2 == 0.0) return 0.0;
+    if (!(r2 < D * D)) return 0.0;                                   // r = 0 (two elements at one point) is a pair like any other here: U_rep(0) = gamma pi R^4, A3
     const double h = D - sqrt(r2);
     return (double)a.gamma * (3.14159265358979323846 / 48.0) * h * h * h * (4.0 * D - h);
 }

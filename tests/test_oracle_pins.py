@@ -548,3 +548,62 @@ def test_a6_population_follows_from_the_rdot_density(small_binary):
     assert cnt.max() <= 64
     inband = np.abs(rd + p["v_dead"]) <= p["tau_s"]                      # NaN (no pair) compares False
     assert np.array_equal(dl > 0, inband.any(1)) and 3 < (dl > 0).sum() < w.n
+
+
+# ------------------------------------------------------------------ round 3: the last unpinned output, A3 in energies, P5 as written
+def test_angular_and_linear_momentum_by_hand():
+    """orc_energy's P and L against numbers worked out by hand (not by conservation, which a flipped sign or a
+    permuted component would survive): m = 2 at x = (1, 2, 3), v = (0.5, -1, 0.25) has x cross v = (3.5, 1.25, -2),
+    m = 3 at x = (-1, 0, 2), v = (0, 1, -1) has x cross v = (-2, -1, -1)."""
+    posm = np.array([[1.0, 2.0, 3.0, 2.0], [-1.0, 0.0, 2.0, 3.0]])
+    vel = np.array([[0.5, -1.0, 0.25, 0.0], [0.0, 1.0, -1.0, 0.0]])
+    p = dict(G=1.0, eps=0.1, dt=1e-3, q=1.0, gamma=0.0, beta=1.0, R_start=(0.0, 0.0), R_end=(0.0, 0.0), n_ramp=0)
+    one = oracle.Sim(posm[:1], vel[:1], np.zeros(1, np.int32), p).energy()
+    assert np.allclose(one["L"], [7.0, 2.5, -4.0], rtol=0, atol=1e-15)
+    assert np.allclose(one["P"], [1.0, -2.0, 0.5], rtol=0, atol=1e-15)
+    both = oracle.Sim(posm, vel, np.array([0, 1], np.int32), p).energy()
+    assert np.allclose(both["L"], [1.0, -0.5, -7.0], rtol=0, atol=1e-15)
+    assert np.allclose(both["P"], [1.0, 1.0, -2.5], rtol=0, atol=1e-15)
+    assert both["KE"] == pytest.approx(0.5 * 2 * (0.25 + 1 + 0.0625) + 0.5 * 3 * 2.0, abs=1e-15)
+
+
+def test_a3_coincident_pair_no_force_but_its_potentials_by_formula():
+    """Reading A3: two distinct elements at one point exert no force on each other (d/r has no
+    direction there), while both potentials are evaluated by their formulas, which are finite at r = 0 when
+    eps > 0: the pair adds -G m_i m_j / eps to U_grav and gamma pi R^4 to U_rep (A12 at r = 0).  With a third
+    element present the coincident two feel only it -- and equally."""
+    posm = np.array([[0.5, -1.0, 2.0, 2.0], [0.5, -1.0, 2.0, 3.0]])
+    vel = np.zeros((2, 4))
+    star = np.zeros(2, np.int32)
+    p = dict(G=1.5, eps=0.25, dt=1e-3, q=1.0, gamma=400.0, beta=0.5, R_start=(0.1, 0.1), R_end=(0.1, 0.1), n_ramp=0)
+    a = oracle.accel(posm, vel, posm[:, 3], star, p["R_start"], p)
+    assert (a == 0).all()
+    e = oracle.Sim(posm, vel, star, p).energy()
+    assert e["Ug"] == pytest.approx(-1.5 * 6.0 / 0.25, rel=1e-15)               # -36
+    assert e["Urep"] == pytest.approx(400.0 * np.pi * float(np.float32(0.1)) ** 4, rel=1e-12)   # the radius is an fp32 model parameter (A8)
+    third = np.array([[0.5, -1.0, 4.0, 1.0]])                                  # 2 above them, out of contact
+    posm3 = np.concatenate([posm, third]); vel3 = np.zeros((3, 4)); star3 = np.zeros(3, np.int32)
+    a3 = oracle.accel(posm3, vel3, posm3[:, 3], star3, p["R_start"], p)
+    g = 1.5 * 1.0 / (2.0 + 0.25) ** 2
+    assert np.allclose(a3[0], [0, 0, g], atol=1e-15) and np.array_equal(a3[0], a3[1])
+    assert np.allclose(a3[2], [0, 0, -1.5 * 5.0 / 2.25 ** 2], atol=1e-15)
+    # eps = 0: the singularity eps exists to remove (PAPER.md:87) -- U_grav of the coincident pair diverges
+    with np.errstate(divide="ignore"):
+        e0 = oracle.Sim(posm, vel, star, dict(p, eps=0.0)).energy()
+    assert e0["Ug"] == -np.inf and (oracle.accel(posm, vel, posm[:, 3], star, p["R_start"], dict(p, eps=0.0)) == 0).all()
+
+
+def test_p5_as_written_config1_thousand_steps():
+    """total momentum and angular momentum of config 1 (N = 2,048, contacts on) over 1,000 leapfrog
+    steps (the integrator is 'conservative'), relative to sum m |v| and |L|, at the 1e-12 the survey states."""
+    w = make_config(1)
+    s = oracle.Sim(w.posm, w.vel, w.star, w.params)
+    e0 = s.energy()
+    pscale = (s.m * np.linalg.norm(s.v, axis=1)).sum()
+    for _ in range(4):
+        s.step(250)
+        e = s.energy()
+        assert np.abs(e["P"] - e0["P"]).max() / pscale < 1e-12
+        assert np.abs(e["L"] - e0["L"]).max() / np.linalg.norm(e0["L"]) < 1e-12
+    assert s.n == 1000
+    assert np.isfinite(e["E"]) and e["E"] < e0["E"]                             # beta < 1: the contacts of the unrelaxed stars dissipate
