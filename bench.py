@@ -177,7 +177,7 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": w.name, "n": w.n, "note": "CPU oracle, bounded sample of the same workload"},
+        "config": workload_config(w, p),
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
                          "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -186,21 +186,46 @@ def run_reference(args):
     return 0
 
 
+def workload_config(w, p):
+    """The `config` object of the JSON line: the same keys and values from both arms (the driver compares them)."""
+    return {"workload": w.name, "n": w.n, "n1": w.meta["n1"], "n2": w.meta["n2"], "q": p["q"],
+            "eps": p["eps"], "dt": p["dt"], "gamma": p["gamma"], "beta": p["beta"],
+            "step": "KDK leapfrog: kick/drift + contact pass (Eqs. 5/6) + all-pairs gravity (Eq. 4) + reduce/kick",
+            "l2": "own arm: flushed between timed steps (256 MiB fill); reference arm (CPU oracle): a bounded sample of "
+                  "i-rows per step, no GPU",
+            "parallelism": "replicas only"}
+
+
 # ----------------------------------------------------------------------------- own arm
+def kernel_source_sha():
+    """sha256 over the kernel sources: a committed ncu capture names the sources it was taken from."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in ("nb_kernels.cuh", "nb_cells.cuh", "nb_fused.cuh", "nb_api.cu"):
+        with open(os.path.join(ROOT, "paper_2303_12166_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
 def profile_traffic(kernel):
-    """(dram bytes per launch, source) from the committed `ncu --set full` summary of THIS kernel instantiation
-    (profiles/r2_gravity_sym_kernel_full.md names the instantiation it captured), else (None, why)."""
-    path = os.path.join(ROOT, "profiles", "r2_gravity_sym_kernel_full.md" if "sym" in kernel else "r1_gravity_kernel_full.md")
+    """(dram bytes per launch, source) from the committed `ncu --set full` summary of THIS kernel instantiation built
+    from THESE sources (profiles/r3_gravity_sym_kernel_full.md carries `kernel = ...`, `kernel_source_sha = ...` and
+    `dram_bytes_per_launch = ...` lines), else (None, why): a capture of older sources is not this run's traffic."""
+    path = os.path.join(ROOT, "profiles", "r3_gravity_sym_kernel_full.md")
     try:
         text = open(path).read()
     except OSError:
         return None, "no committed capture"
     if kernel.replace(" ", "") not in text.replace(" ", ""):
         return None, f"{os.path.basename(path)} is a capture of another kernel instantiation"
+    sha = kernel_source_sha()
+    if f"kernel_source_sha = {sha}" not in text:
+        return None, f"{os.path.basename(path)} was captured from other kernel sources (now {sha}): re-capture"
     for line in text.splitlines():
         if line.startswith("dram_bytes_per_launch"):
             try:
-                return float(line.split("=")[1].split()[0]), f"profiles/{os.path.basename(path)} (ncu --set full, committed)"
+                return float(line.split("=")[1].split()[0]), (f"profiles/{os.path.basename(path)} (ncu --set full of sources "
+                                                               f"{sha}, committed; not measured by this run)")
             except (ValueError, IndexError):
                 break
     return None, "no dram_bytes_per_launch line"
@@ -311,11 +336,11 @@ def run_own(args):
     from workloads import params_f32
 
     rank, local_rank, world = dist_env()
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback "
                          "(use --impl reference for the oracle timing)")
-    if world != args.gpus:
-        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     dist_init("nccl")
@@ -373,21 +398,27 @@ def run_own(args):
     executed = executed_flop_per_interaction(symmetric, info["i_per_cta"], n)
     achieved = executed * int_per_s / 1e12                       # what the ALUs did
     algorithmic = FLOP_PER_INTERACTION * int_per_s / 1e12        # what Eq. 4 needs for the N^2 ordered interactions delivered
-    # pipe occupancy implied by the instruction mix: FP32 lane-operations per interaction on the
-    # 128-lane FMA pipe, MUFU per interaction on the 16-lane XU pipe -- the kernel's real ceilings
-    lane_ops = 7.5 if symmetric else 13.5
-    mufu = 1.0 if symmetric else 1.5
-    clk = sm_max_mhz * 1e6
     traffic, traffic_src = profile_traffic(kernel)
-    nslab = info["j_splits"]
+    # what the launched plan moves per force evaluation besides reading the N positions (ALU-bound: HBM is not the limit)
+    T = info["j_splits"]                    # symmetric: super-tiles; one-sided: j splits
+    ncontact = 1 if (p["gamma"] > 0 and n >= 8192) else 0
+    if "chain" in kernel:                   # no slabs: every CTA adds 2 x S x 3 fp64 sums in place (read + write, L2-resident)
+        traffic_model = {"mode": "chain", "slab_bytes_written": 0.0, "slabs": 0,
+                         "acc64_read_modify_write_bytes": 48.0 * (T + 1) * n, "contact_slab_bytes": 16.0 * ncontact * n,
+                         "note": "T(T+1)/2 CTAs x 2 tiles x S x 24 B read + written in turn order; the update kernel reads "
+                                 "48 B/element of sums + the contact slab"}
+    elif "fused" in kernel:
+        traffic_model = {"mode": "fused", "slab_bytes_written": 0.0, "slabs": 0,
+                         "note": "one cooperative launch: no partial sums in global memory; every CTA re-stages the N "
+                                 "positions (16 B each) per step"}
+    else:
+        traffic_model = {"mode": "slabs", "slab_bytes_written": 16.0 * (T + ncontact) * n, "slabs": T + ncontact,
+                         "note": "partial sums written once per launch and read once by nb_reduce_update_kernel"}
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
                 "frac": achieved / peak_tflops,
                 "achieved_algorithmic": algorithmic, "frac_algorithmic": algorithmic / peak_tflops,
-                "fma_pipe_frac": lane_ops * int_per_s / (sms * 128 * clk),
-                "xu_pipe_frac": mufu * int_per_s / (sms * 16 * clk),
                 "traffic": traffic, "traffic_source": traffic_src,
-                "traffic_model": {"slab_bytes_written": float(nslab) * n * 16, "slabs": nslab,
-                                  "note": "partial sums the kernel writes once per launch (ALU-bound: HBM is not the limit)"},
+                "traffic_model": traffic_model,
                 "kernel": kernel, "kernel_ms": k_ms,
                 **({"kernel_ms_note": "n < 8192: the step runs in ONE cooperative launch (nb_fused_step_kernel); kernel_ms and "
                                       "contact_pass_ms time the stand-alone one-sided gravity kernel and index-order contact "
@@ -398,7 +429,7 @@ def run_own(args):
                 "note": "achieved/frac: FP32 flop the kernel EXECUTES (13.5 per ordered interaction when every unordered "
                         "pair is evaluated once) against the FP32 peak; *_algorithmic: the 21 flop per ordered interaction "
                         "of SURVEY 8(d) x N^2 delivered -- can reach 1 because half of them are never evaluated; "
-                        "fma_pipe_frac / xu_pipe_frac: occupancy of the two pipes that bound the loop",
+                        "pipe occupancies (FMA, XU) are ncu counters, not derived here: profiles/r3_gravity_sym_kernel_full.md",
                 "kernel_share_of_step": k_ms / step_ms,
                 "contact_pass_ms": c_ms, "contact_pass_share_of_step": c_ms / step_ms,
                 "interactions_per_s": int_per_s,
@@ -444,11 +475,8 @@ def run_own(args):
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": step_ms, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": w.name, "n": n, "n1": w.meta["n1"], "n2": w.meta["n2"], "q": p["q"],
-                       "eps": p["eps"], "dt": p["dt"], "gamma": p["gamma"], "beta": p["beta"],
-                       "step": "KDK leapfrog: kick/drift + contact pass (Eqs. 5/6) + all-pairs gravity (Eq. 4) + reduce/kick",
-                       "l2": "flushed between timed steps (256 MiB fill)", "parallelism": "replicas only",
-                       "launch": info},
+            "config": workload_config(w, p),
+            "launch": info,
             "ms_per_step_median": ms_sorted[len(ms_sorted) // 2], "ms_per_step_best": ms_sorted[0],
             "steps_per_s": 1e3 / step_ms,
             "pct_of_fp32_peak": 100.0 * FLOP_PER_INTERACTION * value / world / (peak_tflops * 1e12),
@@ -471,35 +499,10 @@ def run_own(args):
 
 
 # ----------------------------------------------------------------------------- N replicas from one command
-def run_stub(args):
-    """The timing path of run_own with the GPU taken out (gloo, a sleep for a step): lets a CPU-only test drive
-    `main(["--gpus", "2", ...])` through the rank spawning, the barriers and the max-over-ranks."""
-    rank, _, world = dist_env()
-    if world != args.gpus:
-        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}")
-    dist_init("gloo")
-    barrier()
-    ms_local = 0.0
-    for _ in range(args.steps):
-        tt = time.perf_counter()
-        time.sleep(0.002 * (1 + rank))                 # rank 1 is the slower one: the max must pick it
-        ms_local += (time.perf_counter() - tt) * 1e3
-    barrier()
-    ms_total = reduce_over_ranks(ms_local, "max")
-    units = reduce_over_ranks(1000.0 * args.steps, "sum")
-    if rank == 0:
-        print(json.dumps({"impl": "stub", "metric": METRIC, "value": units / (ms_total * 1e-3), "unit": UNIT, "n_gpus": world,
-                          "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_total / args.steps,
-                          "scaling": "weak", "config": {"workload": "stub", "parallelism": "replicas only"}}), flush=True)
-    import torch.distributed as dist
-    if dist.is_initialized():
-        dist.destroy_process_group()
-    return 0
-
-
-def spawn_ranks(args, argv):
+def spawn_ranks(args, argv, script=None):
     """`python bench.py --gpus N` without a launcher: start the N ranks (one process per GPU, RANK / LOCAL_RANK /
-    WORLD_SIZE / MASTER_* set as torchrun would), relay rank 0's line, fail if any rank fails."""
+    WORLD_SIZE / MASTER_* set as torchrun would), relay rank 0's line, fail if any rank fails.  `script`: the file
+    the ranks run (this one)."""
     import socket
     with socket.socket() as sk:
         sk.bind(("127.0.0.1", 0))
@@ -508,7 +511,7 @@ def spawn_ranks(args, argv):
     for r in range(args.gpus):
         env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(args.gpus), MASTER_ADDR="127.0.0.1",
                    MASTER_PORT=str(port))
-        procs.append(subprocess.Popen([sys.executable, os.path.abspath(__file__)] + list(argv), env=env,
+        procs.append(subprocess.Popen([sys.executable, script or os.path.abspath(__file__)] + list(argv), env=env,
                                       stdout=subprocess.PIPE if r == 0 else subprocess.DEVNULL, text=True))
     out, _ = procs[0].communicate()
     rcs = [procs[0].returncode] + [pr.wait() for pr in procs[1:]]
@@ -529,7 +532,7 @@ def main(argv=None):
                     help="scale the element counts of --config (same recipe and seed): for crossover measurements only")
     ap.add_argument("--path", choices=["auto", "one-sided", "symmetric"], default="auto",
                     help="row-a2 kernel (nb_set_force_path); auto = the library's choice")
-    ap.add_argument("--impl", choices=["own", "reference", "stub"], default="own")
+    ap.add_argument("--impl", choices=["own", "reference"], default="own")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle timing leg")
     ap.add_argument("--no-per-config", action="store_true", help="skip the other four configs")
     args = ap.parse_args(argv)
@@ -539,7 +542,7 @@ def main(argv=None):
         return run_reference(args)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         return spawn_ranks(args, argv)
-    return run_stub(args) if args.impl == "stub" else run_own(args)
+    return run_own(args)
 
 
 if __name__ == "__main__":

@@ -68,15 +68,22 @@ def test_two_rank_gloo_timing_reduction(tmp_path):
         assert float(res[3]) == 15.0 and float(res[4]) == 3.0        # max over ranks, sum over ranks
 
 
-def test_gpus_flag_starts_the_ranks_itself():
-    """`python bench.py --gpus 2` with no launcher around it: bench.py starts two ranks (RANK / WORLD_SIZE / MASTER_*
-    as torchrun would), they rendezvous (gloo here: the GPU is taken out of the timing path by --impl stub), the
-    timing is the max over ranks, the units the sum, and rank 0 alone prints, with n_gpus = 2."""
-    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT")}
-    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "stub", "--steps", "4"],
-                         capture_output=True, text=True, env=env, cwd=ROOT, timeout=600)
-    assert out.returncode == 0, out.stderr
-    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+def test_gpus_flag_starts_the_ranks_itself(capfd):
+    """`python bench.py --gpus 2` with no launcher around it: bench.spawn_ranks starts two ranks (RANK / WORLD_SIZE /
+    MASTER_* as torchrun would), they rendezvous (gloo here: the ranks run tests/bench_stub_rank.py, bench.py's timing
+    path with the GPU taken out), the timing is the max over ranks, the units the sum, and rank 0 alone prints, with
+    n_gpus = 2."""
+    import argparse
+    sys.path.insert(0, ROOT)
+    import bench
+    saved = {k: os.environ.pop(k) for k in ("RANK", "LOCAL_RANK", "WORLD_SIZE", "MASTER_ADDR", "MASTER_PORT") if k in os.environ}
+    try:
+        rc = bench.spawn_ranks(argparse.Namespace(gpus=2), ["--gpus", "2", "--steps", "4"],
+                               script=os.path.join(ROOT, "tests", "bench_stub_rank.py"))
+    finally:
+        os.environ.update(saved)
+    assert rc == 0
+    lines = [l for l in capfd.readouterr().out.splitlines() if l.startswith("{")]
     assert len(lines) == 1                                   # rank 0 only
     d = json.loads(lines[0])
     assert d["n_gpus"] == 2 and d["steps"] == 4 and d["config"]["parallelism"] == "replicas only"
@@ -86,6 +93,18 @@ def test_gpus_flag_starts_the_ranks_itself():
 
 def test_gpus_flag_must_agree_with_the_launcher():
     env = dict(os.environ, RANK="0", LOCAL_RANK="0", WORLD_SIZE="1", MASTER_ADDR="127.0.0.1", MASTER_PORT="29618")
-    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--impl", "stub"],
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2"],
                          capture_output=True, text=True, env=env, cwd=ROOT, timeout=600)
     assert out.returncode != 0 and "WORLD_SIZE=1" in (out.stderr + out.stdout)
+
+
+def test_both_arms_print_the_same_config_object():
+    """The driver compares the two arms' `config`: one function makes it for both."""
+    sys.path.insert(0, ROOT)
+    import bench
+    from workloads import make_config, params_f32
+    w = make_config(1)
+    c = bench.workload_config(w, params_f32(w.params))
+    assert c["workload"] == w.name and c["n"] == 2048 and c["parallelism"] == "replicas only" and "flushed" in c["l2"]
+    src = open(os.path.join(ROOT, "bench.py")).read()
+    assert src.count('"config": workload_config(w, p)') == 2
