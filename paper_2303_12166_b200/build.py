@@ -25,20 +25,16 @@ NVCC_FLAGS = [
 ]
 
 
-PROF_LIB = os.path.join(HERE, "libnb_prof.so")     # development build: phase time stamps in nb_fused_step_kernel
-
-
-def build(force: bool = False, verbose: bool = False, prof: bool = False) -> str:
-    """prof=True: the same library with -DNB_FUSED_PROF (see fused_phases.py), as libnb_prof.so; never loaded by default."""
-    lib = PROF_LIB if prof else LIB
+def build(force: bool = False, verbose: bool = False) -> str:
+    lib = LIB
     if not force and os.path.exists(lib) and all(
             os.path.getmtime(lib) >= os.path.getmtime(d) for d in DEPS):
         return lib
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    cmd = [nvcc] + NVCC_FLAGS + (["-DNB_FUSED_PROF"] if prof else []) + (["-Xptxas", "-v"] if verbose else []) + ["-o", lib] + SOURCES
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", lib] + SOURCES
     subprocess.check_call(cmd)
     return lib
 
 
 if __name__ == "__main__":
-    print(build(force=True, verbose="-v" in sys.argv, prof="--prof" in sys.argv))
+    print(build(force=True, verbose="-v" in sys.argv))

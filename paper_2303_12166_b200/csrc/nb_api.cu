@@ -1109,10 +1109,6 @@ int nb_time_contact_pass(nb_ctx* c, int reps, float* ms_avg)
     return time_launches(c, reps, ms_avg, launch_contact);
 }
 
-#ifdef NB_FUSED_PROF
-int nb_debug_fused_prof(long long* host) { return (int)cudaMemcpyFromSymbol(host, nb::g_fused_prof, sizeof(long long) * 512 * 64); }
-#endif
-
 double nb_roche_lobe_radius(double mass_ratio, double k)
 {
     if (!(mass_ratio > 0.0) || !std::isfinite(mass_ratio) || !(k > 0.0)) return NAN;

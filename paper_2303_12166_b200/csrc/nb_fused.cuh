@@ -38,17 +38,6 @@
 
 namespace nb {
 
-#ifdef NB_FUSED_PROF                    // development aid (never defined in the shipped build): phase time stamps
-__device__ long long g_fused_prof[512][64];
-__device__ __forceinline__ void fused_stamp(int& k) {
-    if (threadIdx.x == 0 && k < 64) { long long t; asm volatile("mov.u64 %0, %globaltimer;" : "=l"(t)); g_fused_prof[blockIdx.x][k] = t; }
-    ++k;
-}
-#define NB_STAMP() fused_stamp(prof_k)
-#else
-#define NB_STAMP()
-#endif
-
 constexpr int kFusedGroup = 8;                     // elements j per group: four Montgomery pairs in flight per thread
 constexpr int kFusedThreads = 512;                 // 16 warps: four per SM sub-partition
 constexpr int kFusedWarps = kFusedThreads / 32;
@@ -150,10 +139,6 @@ nb_fused_step_kernel(const __grid_constant__ FusedArgs f)
     const long long step0 = f.dev->step, n_ramp = f.dev->n_ramp;
     const double Rs0 = f.dev->R_start[0], Rs1 = f.dev->R_start[1], Re0 = f.dev->R_end[0], Re1 = f.dev->R_end[1];
     long long nstep = step0;
-#ifdef NB_FUSED_PROF
-    int prof_k = 0;
-#endif
-    NB_STAMP();
 
     // where the state is (read) and where the next update puts it
     float4 *xs = f.posm, *vs = f.vel, *xd = f.posm2, *vd = f.vel2;
@@ -184,9 +169,7 @@ nb_fused_step_kernel(const __grid_constant__ FusedArgs f)
         }
         if (across) swap_buffers();
         ++nstep;
-        NB_STAMP();
         grid.sync();
-        NB_STAMP();
     }
 
     const int ngroups = f.npad / kFusedGroup;
@@ -219,7 +202,6 @@ nb_fused_step_kernel(const __grid_constant__ FusedArgs f)
             }
         }
         __syncthreads();
-        NB_STAMP();
 
         // F: gravity over the thread's groups of elements j, contact candidates queued
         const float4 pa = sx[i0], pb = sx[i1];
@@ -279,7 +261,6 @@ nb_fused_step_kernel(const __grid_constant__ FusedArgs f)
             if ((k & (kFusedFlush - 1)) == kFusedFlush - 1) flush();
         }
         flush();
-        NB_STAMP();
 
         if (contact) {
             // the warp's queued pairs dealt evenly to its lanes -- a lane with 6 pairs no longer holds up 31 lanes
@@ -318,7 +299,6 @@ nb_fused_step_kernel(const __grid_constant__ FusedArgs f)
                 __syncwarp();
             }
         }
-        NB_STAMP();
 
         // R: sum over the segments.  Lanes with the same pair index: xor butterfly (the same tree in every lane,
         // operands commuted: the same bits); then the CTA's 16 warps in warp order.
@@ -361,9 +341,7 @@ nb_fused_step_kernel(const __grid_constant__ FusedArgs f)
         if (!last) {
             swap_buffers();
             ++nstep;
-            NB_STAMP();
             grid.sync();
-            NB_STAMP();
         }
     }
     if (blockIdx.x == 0 && tid == 0 && nstep != step0) set_step(f.dev, nstep);
