@@ -130,8 +130,17 @@ int nb_relax(nb_ctx* ctx, int nsteps, float kappa);
  *   [12..14] Ldisk0 [15..17] Ldisk1   angular momentum of the Min_s elements about the other star,
  *                                     sum m (x - X_o) x (v - V_o)
  *   [30] step count, [31] 0.
- * All sums and decisions in fp64 on the fp32 state.  Synchronises the stream (twice). */
+ * All sums and decisions in fp64 on the fp32 state, all of them on the device (star centres, the L1 plane by
+ * Newton iteration on the force balance, Eq. 3); the record is then copied to the host.  Synchronises the stream. */
 int nb_transfer_diagnostics(nb_ctx* ctx, double k_lobe, double* out);
+
+/* f3 per step, on the device ("donor mass beyond the L1 plane / inside the accretor's lobe per step";
+ * PAPER.md:15, 107-109): the same 32-double record, written to row n of dev_series[rows][32] (DEVICE memory,
+ * caller-owned, 8-byte aligned), n = the run's step count when the launches execute; a run past the last row
+ * (n >= rows) writes nothing.  Four short launches on the ctx stream, no host synchronisation: call it after
+ * nb_step(1) in a loop (or capture the pair in a CUDA graph) and read the series back once at the end.
+ * Rows the run did not visit keep whatever the caller put there. */
+int nb_transfer_record(nb_ctx* ctx, double k_lobe, double* dev_series, int64_t rows);
 
 /* f4, headless point splat in place of the paper's OpenGL viewer (reading A19):
  * orthographic projection of the element positions on coordinate axes (axis_u, axis_v in {0,1,2},

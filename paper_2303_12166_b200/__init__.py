@@ -19,7 +19,7 @@ NB_OK, NB_EINVAL, NB_ESTATE, NB_ECUDA, NB_ENOMEM, NB_EARCH, NB_ESIZE = 0, -1, -2
 NB_PATH_AUTO, NB_PATH_ONE_SIDED, NB_PATH_SYMMETRIC = 0, 1, 2
 
 EXPORTS = ("nb_create", "nb_workspace_bytes", "nb_set_state", "nb_compute_accel", "nb_step",
-           "nb_energy", "nb_set_step", "nb_relax", "nb_transfer_diagnostics", "nb_splat", "nb_get_step", "nb_upload_state",
+           "nb_energy", "nb_set_step", "nb_relax", "nb_transfer_diagnostics", "nb_transfer_record", "nb_splat", "nb_get_step", "nb_upload_state",
            "nb_download_state",
            "nb_get_launch_info", "nb_set_force_path", "nb_force_kernel_name", "nb_launch_count",
            "nb_time_force_kernel", "nb_time_contact_pass", "nb_contact_stats", "nb_destroy", "nb_strerror",
@@ -75,6 +75,8 @@ def lib() -> C.CDLL:
         L.nb_relax.argtypes = [vp, C.c_int, C.c_float]
         L.nb_transfer_diagnostics.restype = C.c_int
         L.nb_transfer_diagnostics.argtypes = [vp, C.c_double, C.POINTER(C.c_double)]
+        L.nb_transfer_record.restype = C.c_int
+        L.nb_transfer_record.argtypes = [vp, C.c_double, vp, i64]
         L.nb_splat.restype = C.c_int
         L.nb_splat.argtypes = [vp, C.POINTER(C.c_float), C.c_float, C.c_int, C.c_int, C.c_int, C.c_int, vp]
         L.nb_get_step.restype = C.c_int
@@ -195,6 +197,17 @@ def nb_transfer_diagnostics(ctx: int, k_lobe: float = 0.6) -> Dict[str, object]:
     return dict(M0=v[0], M1=v[1], a=v[2], d0=v[3], rL0=v[4], rL1=v[5], Mcross0=v[6], Mcross1=v[7],
                 Min0=v[8], Min1=v[9], Mout0=v[10], Mout1=v[11], Ldisk=[v[12:15], v[15:18]],
                 X=[v[18:21], v[21:24]], V=[v[24:27], v[27:30]], step=int(v[30]))
+
+
+TRANSFER_RECORD = ("M0", "M1", "a", "d0", "rL0", "rL1", "Mcross0", "Mcross1", "Min0", "Min1", "Mout0", "Mout1")   # columns 0..11
+
+
+def nb_transfer_record(ctx: int, k_lobe: float, dev_series, rows: Optional[int] = None) -> None:
+    """The record of nb_transfer_diagnostics into row `step count` of the DEVICE array dev_series [rows][32] (float64);
+    asynchronous, no host synchronisation."""
+    if rows is None:
+        rows = dev_series.shape[0]
+    _check(lib().nb_transfer_record(ctx, float(k_lobe), _ptr(dev_series), int(rows)), "nb_transfer_record", ctx)
 
 
 def nb_splat(ctx: int, centre: Sequence[float], half_width: float, axis_u: int, axis_v: int, W: int, H: int,
@@ -347,6 +360,9 @@ class Simulation:
 
     def transfer_diagnostics(self, k_lobe: float = 0.6) -> Dict[str, object]:
         return nb_transfer_diagnostics(self.ctx, k_lobe)
+
+    def transfer_record(self, series, k_lobe: float = 0.6) -> None:
+        nb_transfer_record(self.ctx, k_lobe, series)
 
     def splat(self, centre, half_width: float, axis_u: int = 0, axis_v: int = 1, W: int = 512, H: int = 512):
         with self.torch.cuda.stream(self.stream):

@@ -151,7 +151,7 @@ Plan make_plan(int64_t n, int num_sms, int path)
 
 struct Layout {
     size_t off_dev, off_acc, off_part, off_red, off_ps, off_vs, off_gbox, off_sbox, off_cpart, off_cstate,
-        off_counters, off_bsum, off_bucket, off_slot, off_tmp, off_perm, off_acc64, off_turn, off_epot, off_erep, off_tbox, total;
+        off_counters, off_bsum, off_bucket, off_slot, off_tmp, off_perm, off_acc64, off_turn, off_epot, off_erep, off_tbox, off_xfer, total;
 };
 
 // Super-tile of nb_pot_pair_kernel for n elements (T <= 512 up to 2M elements), and its CTAs = fp64 partials.
@@ -191,6 +191,7 @@ Layout make_layout(int64_t n_max)
     L.off_epot = o;     o += align_up((size_t)pot_pairs(n_max) * sizeof(double));
     L.off_erep = o;     o += align_up(((size_t)n_max * 4 / kCcThreads + 1) * sizeof(double));
     L.off_tbox = o;     o += align_up(((size_t)n_max / 1024 + 1) * 2 * sizeof(float4));   // nb_energy: boxes of its super-tiles (S >= 1,024)
+    L.off_xfer = o;     o += align_up(sizeof(XferGeom)) + align_up(32 * sizeof(double));   // f3: geometry between the passes, and the record of nb_transfer_diagnostics
     L.total = o;
     return L;
 }
@@ -777,59 +778,42 @@ int nb_relax(nb_ctx* c, int nsteps, float kappa)
     return NB_OK;
 }
 
+// f3 on the device: pass 1 (star moments), geometry (centres, L1 plane, Eq. 3 lobes), pass 2 (decisions), record.
+// Four launches on the ctx stream, nothing synchronises.
+static int launch_transfer(nb_ctx* c, double k_lobe, double* series, long long rows)
+{
+    const int n = (int)c->n;
+    double* red = c->red();
+    XferGeom* g = c->at<XferGeom>(c->lay.off_xfer);
+    nb_star_moments_kernel<<<kMomentBlocks, 256, 0, c->stream>>>(c->posm, c->vel, n, c->n1, red);
+    nb_transfer_geometry_kernel<<<1, 32, 0, c->stream>>>(red, kMomentBlocks, k_lobe, c->dev(), series, rows, g);
+    XferArgs xa;
+    xa.posm = c->posm; xa.vel = c->vel; xa.g = g; xa.out = red; xa.n = n; xa.n1 = c->n1;
+    nb_transfer_kernel<<<kMomentBlocks, 256, 0, c->stream>>>(xa);
+    nb_transfer_finish_kernel<<<1, 32, 0, c->stream>>>(red, kMomentBlocks, g);
+    c->launches += 4;
+    NB_CUDA(c, cudaGetLastError());
+    return NB_OK;
+}
+
 int nb_transfer_diagnostics(nb_ctx* c, double k_lobe, double* out)
 {
     if (!c || !out || !(k_lobe > 0.0) || !std::isfinite(k_lobe)) return NB_EINVAL;
     if (!c->have_state) return NB_ESTATE;
     if (int rc_ = device_guard(c)) return rc_;
-    const int n = (int)c->n;
-    double* red = c->red();
-    double h1[kMomentBlocks * kXferCols1], h2[kMomentBlocks * kXferCols2];
-    nb_star_moments_kernel<<<kMomentBlocks, 256, 0, c->stream>>>(c->posm, c->vel, n, c->n1, red);
-    c->launches++;
-    NB_CUDA(c, cudaGetLastError());
-    DevState hs;
-    NB_CUDA(c, cudaMemcpyAsync(h1, red, sizeof(h1), cudaMemcpyDeviceToHost, c->stream));
-    NB_CUDA(c, cudaMemcpyAsync(&hs, c->dev(), sizeof(hs), cudaMemcpyDeviceToHost, c->stream));
+    double* row = reinterpret_cast<double*>(c->ws + c->lay.off_xfer + align_up(sizeof(XferGeom)));
+    if (int rc = launch_transfer(c, k_lobe, row, -1)) return rc;
+    NB_CUDA(c, cudaMemcpyAsync(out, row, 32 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     NB_CUDA(c, cudaStreamSynchronize(c->stream));
-    double q[kXferCols1] = {0};
-    for (int b = 0; b < kMomentBlocks; ++b)
-        for (int k = 0; k < kXferCols1; ++k) q[k] += h1[b * kXferCols1 + k];
-    for (int k = 0; k < 32; ++k) out[k] = 0.0;
-    const double M0 = q[0], M1 = q[7];
-    out[0] = M0; out[1] = M1; out[30] = (double)hs.step;
-    XferArgs xa;
-    for (int s = 0; s < 2; ++s) {
-        const double M = s ? M1 : M0;
-        for (int k = 0; k < 3; ++k) {
-            xa.X[s][k] = M > 0.0 ? q[7 * s + 1 + k] / M : 0.0;
-            xa.V[s][k] = M > 0.0 ? q[7 * s + 4 + k] / M : 0.0;
-            out[18 + 3 * s + k] = xa.X[s][k];
-            out[24 + 3 * s + k] = xa.V[s][k];
-        }
-    }
-    if (!(M0 > 0.0 && M1 > 0.0)) return NB_OK;                 // one star only: nothing to transfer
-    double d[3], a2 = 0.0;
-    for (int k = 0; k < 3; ++k) { d[k] = xa.X[1][k] - xa.X[0][k]; a2 += d[k] * d[k]; }
-    const double a = std::sqrt(a2);
-    if (!(a > 0.0)) return NB_OK;
-    for (int k = 0; k < 3; ++k) xa.e[k] = d[k] / a;
-    // L1 along the line of centres, measured from star 0 (nb_l1_distance is measured from the primary)
-    xa.d0 = M1 <= M0 ? a * nb_l1_distance(M1 / M0) : a * (1.0 - nb_l1_distance(M0 / M1));
-    xa.rL[0] = a * nb_roche_lobe_radius(M0 / M1, k_lobe);      // Eq. 3: the star's own mass in the numerator
-    xa.rL[1] = a * nb_roche_lobe_radius(M1 / M0, k_lobe);
-    xa.posm = c->posm; xa.vel = c->vel; xa.out = red; xa.n = n; xa.n1 = c->n1;
-    nb_transfer_kernel<<<kMomentBlocks, 256, 0, c->stream>>>(xa);
-    c->launches++;
-    NB_CUDA(c, cudaGetLastError());
-    NB_CUDA(c, cudaMemcpyAsync(h2, red, sizeof(h2), cudaMemcpyDeviceToHost, c->stream));
-    NB_CUDA(c, cudaStreamSynchronize(c->stream));
-    double r[kXferCols2] = {0};
-    for (int b = 0; b < kMomentBlocks; ++b)
-        for (int k = 0; k < kXferCols2; ++k) r[k] += h2[b * kXferCols2 + k];
-    out[2] = a; out[3] = xa.d0; out[4] = xa.rL[0]; out[5] = xa.rL[1];
-    for (int k = 0; k < kXferCols2; ++k) out[6 + k] = r[k];    // Mcross[2], Min[2], Mout[2], Ldisk[2][3]
     return NB_OK;
+}
+
+int nb_transfer_record(nb_ctx* c, double k_lobe, double* dev_series, int64_t rows)
+{
+    if (!c || !dev_series || rows < 1 || ((uintptr_t)dev_series & 7) || !(k_lobe > 0.0) || !std::isfinite(k_lobe)) return NB_EINVAL;
+    if (!c->have_state) return NB_ESTATE;
+    if (int rc_ = device_guard(c)) return rc_;
+    return launch_transfer(c, k_lobe, dev_series, (long long)rows);
 }
 
 int nb_splat(nb_ctx* c, const float* centre, float half_width, int axis_u, int axis_v, int W, int H,

@@ -1483,44 +1483,141 @@ nb_star_moments_kernel(const float4* __restrict__ posm, const float4* __restrict
     }
 }
 
+// Between the passes, on the device (so a record per step needs no host round trip): star centres and masses from
+// pass 1's block partials (summed in block order), the L1 plane by the force balance along the line of centres
+// (Newton iteration, as nb_l1_distance() on the host), the lobe radii by Eq. 3.
+struct XferGeom {
+    double X[2][3], V[2][3], e[3], d0, rL[2], a, M[2];
+    double* out;                       // the 32-double record this evaluation writes (null: dropped)
+    long long step;
+    int valid;                         // both stars present and apart: pass 2 has something to decide
+};
+
+__device__ inline double dev_l1_distance(double q)            // distance of L1 from the primary, separation 1, q = m2/m1 <= 1
+{
+    const double mu2 = q / (1.0 + q), mu1 = 1.0 - mu2;
+    double s = 1.0 - cbrt(mu2 / 3.0);
+    for (int it = 0; it < 100; ++it) {
+        const double t = 1.0 - s;
+        const double f = -mu1 / (s * s) + mu2 / (t * t) + (s - mu2);
+        const double df = 2.0 * mu1 / (s * s * s) + 2.0 * mu2 / (t * t * t) + 1.0;
+        const double sn = s - f / df;
+        if (!(sn > 0.0 && sn < 1.0)) { s = 0.5 * (s + (sn <= 0.0 ? 0.0 : 1.0)); continue; }
+        if (fabs(sn - s) < 1e-15) { s = sn; break; }
+        s = sn;
+    }
+    return s;
+}
+
+__device__ inline double dev_roche_lobe_radius(double mass_ratio, double k)
+{
+    const double c = cbrt(mass_ratio);
+    return 0.49 * c * c / (k * c * c + log1p(c));                // Eq. 3
+}
+
+// rows < 0: the record goes to series[0..31]; else to row `step count` of series[rows][32], dropped when the run is past it.
+__global__ void __launch_bounds__(32)
+nb_transfer_geometry_kernel(const double* __restrict__ part1 /*[blocks][14]*/, int blocks, double k_lobe,
+                            const DevState* __restrict__ dev, double* series, long long rows, XferGeom* __restrict__ g)
+{
+    __shared__ double q[kXferCols1];
+    const int t = threadIdx.x;
+    if (t < kXferCols1) {
+        double sum = 0.0;
+        for (int b = 0; b < blocks; ++b) sum += part1[(size_t)b * kXferCols1 + t];
+        q[t] = sum;
+    }
+    __syncthreads();
+    if (t != 0) return;
+    const long long step = dev->step;
+    double* out = rows < 0 ? series : (step < rows ? series + 32 * step : nullptr);
+    g->out = out; g->step = step; g->valid = 0;
+    const double M0 = q[0], M1 = q[7];
+    g->M[0] = M0; g->M[1] = M1;
+    for (int s = 0; s < 2; ++s) {
+        const double M = s ? M1 : M0;
+        for (int k = 0; k < 3; ++k) {
+            g->X[s][k] = M > 0.0 ? q[7 * s + 1 + k] / M : 0.0;
+            g->V[s][k] = M > 0.0 ? q[7 * s + 4 + k] / M : 0.0;
+        }
+    }
+    g->a = 0.0; g->d0 = 0.0; g->rL[0] = g->rL[1] = 0.0; g->e[0] = g->e[1] = g->e[2] = 0.0;
+    if (!(M0 > 0.0 && M1 > 0.0)) return;                         // one star only: nothing to transfer
+    double d[3], a2 = 0.0;
+    for (int k = 0; k < 3; ++k) { d[k] = g->X[1][k] - g->X[0][k]; a2 += d[k] * d[k]; }
+    const double a = sqrt(a2);
+    if (!(a > 0.0)) return;
+    for (int k = 0; k < 3; ++k) g->e[k] = d[k] / a;
+    g->a = a;
+    // L1 along the line of centres, measured from star 0 (dev_l1_distance is measured from the primary)
+    g->d0 = M1 <= M0 ? a * dev_l1_distance(M1 / M0) : a * (1.0 - dev_l1_distance(M0 / M1));
+    g->rL[0] = a * dev_roche_lobe_radius(M0 / M1, k_lobe);       // Eq. 3: the star's own mass in the numerator
+    g->rL[1] = a * dev_roche_lobe_radius(M1 / M0, k_lobe);
+    g->valid = 1;
+}
+
 // Pass 2: every decision in fp64 on the fp32 coordinates.
 struct XferArgs {
     const float4* __restrict__ posm;
     const float4* __restrict__ vel;
+    const XferGeom* __restrict__ g;
     double* __restrict__ out;          // [grid][12]
     int n, n1;
-    double X[2][3], V[2][3], e[3], d0, rL[2];
 };
 
 __global__ void __launch_bounds__(256)
 nb_transfer_kernel(const __grid_constant__ XferArgs a)
 {
     __shared__ double sh[8];
+    __shared__ XferGeom g;
+    if (threadIdx.x == 0) g = *a.g;
+    __syncthreads();
     double q[kXferCols2];
     for (int c = 0; c < kXferCols2; ++c) q[c] = 0.0;
-    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < a.n; i += gridDim.x * blockDim.x) {
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; g.valid && i < a.n; i += gridDim.x * blockDim.x) {
         const float4 p = a.posm[i], v = a.vel[i];
         const int s = i < a.n1 ? 0 : 1, o = 1 - s;
         const double m = p.w;
-        const double x0 = (double)p.x - a.X[0][0], y0 = (double)p.y - a.X[0][1], z0 = (double)p.z - a.X[0][2];
-        const double x1 = (double)p.x - a.X[1][0], y1 = (double)p.y - a.X[1][1], z1 = (double)p.z - a.X[1][2];
-        const double u = x0 * a.e[0] + y0 * a.e[1] + z0 * a.e[2];
+        const double x0 = (double)p.x - g.X[0][0], y0 = (double)p.y - g.X[0][1], z0 = (double)p.z - g.X[0][2];
+        const double x1 = (double)p.x - g.X[1][0], y1 = (double)p.y - g.X[1][1], z1 = (double)p.z - g.X[1][2];
+        const double u = x0 * g.e[0] + y0 * g.e[1] + z0 * g.e[2];
         const double r0 = sqrt(x0 * x0 + y0 * y0 + z0 * z0), r1 = sqrt(x1 * x1 + y1 * y1 + z1 * z1);
-        if (s == 0 ? (u > a.d0) : (u < a.d0)) q[s] += m;                       // beyond the L1 plane
-        if ((o == 0 ? r0 : r1) < a.rL[o]) {                                    // inside the other star's lobe sphere
+        if (s == 0 ? (u > g.d0) : (u < g.d0)) q[s] += m;                       // beyond the L1 plane
+        if ((o == 0 ? r0 : r1) < g.rL[o]) {                                    // inside the other star's lobe sphere
             q[2 + s] += m;
             const double rx = o == 0 ? x0 : x1, ry = o == 0 ? y0 : y1, rz = o == 0 ? z0 : z1;
-            const double wx = (double)v.x - a.V[o][0], wy = (double)v.y - a.V[o][1], wz = (double)v.z - a.V[o][2];
+            const double wx = (double)v.x - g.V[o][0], wy = (double)v.y - g.V[o][1], wz = (double)v.z - g.V[o][2];
             q[6 + 3 * s] += m * (ry * wz - rz * wy);
             q[7 + 3 * s] += m * (rz * wx - rx * wz);
             q[8 + 3 * s] += m * (rx * wy - ry * wx);
         }
-        if (r0 > a.rL[0] && r1 > a.rL[1]) q[4 + s] += m;                       // outside both
+        if (r0 > g.rL[0] && r1 > g.rL[1]) q[4 + s] += m;                       // outside both
     }
     for (int c = 0; c < kXferCols2; ++c) {
         const double r = block_sum(q[c], sh);
         if (threadIdx.x == 0) a.out[(size_t)blockIdx.x * kXferCols2 + c] = r;
     }
+}
+
+// The record (layout: nb.h, nb_transfer_diagnostics): pass 2's block partials summed in block order.
+__global__ void __launch_bounds__(32)
+nb_transfer_finish_kernel(const double* __restrict__ part2 /*[blocks][12]*/, int blocks, const XferGeom* __restrict__ g)
+{
+    double* out = g->out;
+    if (!out) return;
+    const int t = threadIdx.x;
+    double v = 0.0;
+    if (t == 0) v = g->M[0];
+    else if (t == 1) v = g->M[1];
+    else if (t == 2) v = g->a;
+    else if (t == 3) v = g->d0;
+    else if (t == 4) v = g->rL[0];
+    else if (t == 5) v = g->rL[1];
+    else if (t < 6 + kXferCols2) { for (int b = 0; b < blocks; ++b) v += part2[(size_t)b * kXferCols2 + (t - 6)]; }
+    else if (t < 24) v = g->X[(t - 18) / 3][(t - 18) % 3];
+    else if (t < 30) v = g->V[(t - 24) / 3][(t - 24) % 3];
+    else if (t == 30) v = (double)g->step;
+    out[t] = v;
 }
 
 // ---------------------------------------------------------------------------
