@@ -395,3 +395,32 @@ def test_transfer_record_in_a_cuda_graph_and_past_the_last_row(nb):
     assert L.nb_transfer_record(cap.ctx, 0.6, sc.data_ptr(), 0) == nb.NB_EINVAL
     assert L.nb_transfer_record(cap.ctx, -1.0, sc.data_ptr(), 4) == nb.NB_EINVAL
     eager.close(); cap.close()
+
+
+def test_transfer_series_of_the_full_config3_run(nb):
+    """SURVEY 8(f) f3 on BASELINE's config 3 (N = 65,536, 1,000 steps, the donor's radius ramped to its Roche lobe,
+    PAPER.md:89, 107-109): one record per step, nothing synchronising until the end.  The series is complete and
+    consistent -- step column, constant star masses, the last row equal to the host call -- and the donor's mass beyond
+    the L1 plane at the end of the ramp is at least what it was at the start.  Prints the series at every 100th step."""
+    import torch
+    w = make_config(3)
+    p = params_f32(w.params)
+    nsteps = w.meta["nsteps"]
+    s = nb.Simulation(w.posm, w.vel, w.star, p)
+    series = torch.full((nsteps + 1, 32), float("nan"), dtype=torch.float64, device=s.device)
+    s.transfer_record(series)
+    for _ in range(nsteps):
+        s.step(1)
+        s.transfer_record(series)
+    s.synchronize()
+    rec = series.cpu().numpy()
+    last = s.transfer_diagnostics()
+    s.close()
+    assert np.isfinite(rec).all() and np.array_equal(rec[:, 30], np.arange(nsteps + 1))
+    assert np.allclose(rec[:, 0], rec[0, 0], rtol=1e-12, atol=0) and np.allclose(rec[:, 1], rec[0, 1], rtol=1e-12, atol=0)
+    assert rec[-1, 6] == last["Mcross0"] and rec[-1, 8] == last["Min0"] and rec[-1, 2] == last["a"]
+    assert rec[-1, 6] >= rec[0, 6]
+    assert (np.abs(np.diff(rec[:, 2])) < 1e-3 * rec[0, 2]).all()                     # the separation moves smoothly
+    for n in range(0, nsteps + 1, 100):
+        print(f"TRANSFER config3 step={n} a={rec[n, 2]:.6f} d0={rec[n, 3]:.6f} rL0={rec[n, 4]:.6f} "
+              f"Mcross0={rec[n, 6]:.6e} Min0={rec[n, 8]:.6e} Mout0={rec[n, 10]:.6e}")
